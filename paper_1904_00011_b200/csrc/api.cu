@@ -1,0 +1,414 @@
+// api.cu -- the C ABI of include/pcmd.h: argument checks, ctx ownership, launch sequencing.
+// No arithmetic of the method runs on the host: the host only validates, sizes scratch and
+// enqueues kernels.
+#include <math.h>
+#include <stdlib.h>
+#include <string.h>
+#include <new>
+#include "pcmd_internal.cuh"
+
+static uint64_t splitmix64_host(uint64_t j) {  // R-C4 checksum multiplier (debug counts only)
+    uint64_t z = j + 0x9E3779B97F4A7C15ull;
+    z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ull;
+    z = (z ^ (z >> 27)) * 0x94D049BB133111EBull;
+    return z ^ (z >> 31);
+}
+
+template <typename T>
+static int upload(pcmd_ctx *c, T **dst, const T *src, size_t n) {
+    PCMD_CUDA(c, cudaMalloc((void **)dst, (n ? n : 1) * sizeof(T)));
+    if (n) PCMD_CUDA(c, cudaMemcpy(*dst, src, n * sizeof(T), cudaMemcpyHostToDevice));
+    return PCMD_OK;
+}
+
+extern "C" const char *pcmd_strerror(int code) {
+    switch (code) {
+        case PCMD_OK: return "ok";
+        case PCMD_EINVAL: return "invalid argument";
+        case PCMD_ERANGE: return "expected star count of an isochrone point exceeds 2^22";
+        case PCMD_ENOMEM: return "out of memory";
+        case PCMD_ECUDA: return "CUDA error";
+        default: return "unknown error";
+    }
+}
+
+static void free_scratch(pcmd_ctx *c) {
+    cudaFree(c->d_sfh); cudaFree(c->d_model); cudaFree(c->d_mdfw); cudaFree(c->d_lambda);
+    cudaFree(c->d_rawcnt); cudaFree(c->d_klo); cudaFree(c->d_q); cudaFree(c->d_stcnt);
+    cudaFree(c->d_tab); cudaFree(c->d_rec); cudaFree(c->d_fdust);
+    if (c->h_stage) cudaFreeHost(c->h_stage);
+    c->d_sfh = nullptr; c->d_model = nullptr; c->d_mdfw = nullptr; c->d_lambda = nullptr;
+    c->d_rawcnt = nullptr; c->d_klo = nullptr; c->d_q = nullptr; c->d_stcnt = nullptr;
+    c->d_tab = nullptr; c->d_rec = nullptr; c->d_fdust = nullptr; c->h_stage = nullptr;
+    c->cap_models = 0; c->cap_raw = 0;
+}
+
+// Scratch for n_models models whose sampler tables need at most cap_raw raw entries each.
+static int ensure_scratch(pcmd_ctx *c, int n_models, int64_t cap_raw) {
+    if (n_models <= c->cap_models && cap_raw <= c->cap_raw) return PCMD_OK;
+    const int nm = n_models > c->cap_models ? n_models : c->cap_models;
+    const int64_t cr = cap_raw > c->cap_raw ? cap_raw : c->cap_raw;
+    cudaDeviceSynchronize();
+    free_scratch(c);
+    const size_t J = c->J, Jp = c->Jpad;
+    PCMD_CUDA(c, cudaMalloc(&c->d_sfh, (size_t)nm * c->A * sizeof(double)));
+    PCMD_CUDA(c, cudaMalloc(&c->d_model, (size_t)nm * sizeof(DevModel)));
+    PCMD_CUDA(c, cudaMalloc(&c->d_mdfw, (size_t)nm * c->Z * sizeof(double)));
+    PCMD_CUDA(c, cudaMalloc(&c->d_lambda, (size_t)nm * J * sizeof(double)));
+    PCMD_CUDA(c, cudaMalloc(&c->d_rawcnt, (size_t)nm * (J + 1) * sizeof(uint32_t)));
+    PCMD_CUDA(c, cudaMalloc(&c->d_stcnt, (size_t)nm * (J + 1) * sizeof(uint32_t)));
+    PCMD_CUDA(c, cudaMalloc(&c->d_klo, (size_t)nm * J * sizeof(uint32_t)));
+    PCMD_CUDA(c, cudaMalloc(&c->d_q, (size_t)nm * cr * sizeof(double)));
+    PCMD_CUDA(c, cudaMalloc(&c->d_tab, (size_t)nm * cr * sizeof(uint32_t)));
+    PCMD_CUDA(c, cudaMalloc(&c->d_rec, (size_t)nm * Jp * sizeof(PointRec)));
+    PCMD_CUDA(c, cudaMalloc(&c->d_fdust, (size_t)nm * c->B * c->P * sizeof(float)));
+    c->h_stage_bytes = (size_t)nm * (c->A * sizeof(double) + sizeof(DevModel));
+    PCMD_CUDA(c, cudaMallocHost(&c->h_stage, c->h_stage_bytes));
+    c->cap_models = nm; c->cap_raw = cr;
+    return PCMD_OK;
+}
+
+extern "C" int pcmd_create(pcmd_ctx **out, const pcmd_config *cfg) {
+    if (!out || !cfg) return PCMD_EINVAL;
+    *out = nullptr;
+    if (cfg->n_im < 1 || cfg->n_im > 32768 || cfg->n_bands < 1 || cfg->n_bands > PCMD_MAX_BANDS ||
+        cfg->n_age < 1 || cfg->n_feh < 1 || cfg->n_points < 1 || cfg->psf_k < 1 || cfg->psf_k > 63 ||
+        (cfg->psf_k & 1) == 0 || cfg->n_hess < 0 || cfg->n_hess > PCMD_MAX_HESS ||
+        cfg->dust_mode < 0 || cfg->dust_mode > 2)
+        return PCMD_EINVAL;
+    if (!cfg->age_idx || !cfg->feh_idx || !cfg->imf_w || !cfg->absmag || !cfg->feh_grid || !cfg->zp ||
+        !cfg->dust_coef || !cfg->psf || !cfg->sky || !cfg->read_sigma || (cfg->n_hess && !cfg->hess))
+        return PCMD_EINVAL;
+    if (!(cfg->dust_frac >= 0.0 && cfg->dust_frac <= 1.0) || !(cfg->mdf_cut >= 0.0 && cfg->mdf_cut < 1.0) ||
+        !(cfg->like_floor > 0.0))
+        return PCMD_EINVAL;
+    const int J = cfg->n_points, B = cfg->n_bands, K = cfg->psf_k;
+    for (int j = 0; j < J; ++j) {
+        if (cfg->age_idx[j] < 0 || cfg->age_idx[j] >= cfg->n_age || cfg->feh_idx[j] < 0 ||
+            cfg->feh_idx[j] >= cfg->n_feh || !(cfg->imf_w[j] >= 0.0) || !isfinite(cfg->imf_w[j]))
+            return PCMD_EINVAL;
+        for (int b = 0; b < B; ++b) if (!isfinite(cfg->absmag[(size_t)j * B + b])) return PCMD_EINVAL;
+    }
+    for (int b = 0; b < B; ++b)
+        if (!isfinite(cfg->zp[b]) || !(cfg->sky[b] >= 0.0) || cfg->sky[b] > PCMD_LAMBDA_MAX ||
+            !(cfg->read_sigma[b] >= 0.0) || !isfinite(cfg->dust_coef[b]))
+            return PCMD_EINVAL;
+    int64_t bins = 0;
+    for (int h = 0; h < cfg->n_hess; ++h) {
+        const pcmd_hess_spec &s = cfg->hess[h];
+        if (s.band_plus < 0 || s.band_plus >= B || s.band_minus < 0 || s.band_minus >= B || s.band_y < 0 ||
+            s.band_y >= B || s.nx < 1 || s.ny < 1 || s.nx > 4096 || s.ny > 4096 || !(s.x_hi > s.x_lo) ||
+            !(s.y_hi > s.y_lo))
+            return PCMD_EINVAL;
+        bins += (int64_t)s.nx * s.ny;
+    }
+    pcmd_ctx *c = new (std::nothrow) pcmd_ctx;
+    if (!c) return PCMD_ENOMEM;
+    memset(c, 0, sizeof(*c));
+    c->N = cfg->n_im; c->B = B; c->A = cfg->n_age; c->Z = cfg->n_feh; c->J = J; c->Jpad = (J + 3) & ~3;
+    c->K = K; c->psf_sep = cfg->psf_separable; c->shot_noise = cfg->shot_noise != 0;
+    c->poisson_sky = cfg->poisson_sky != 0; c->n_hess = cfg->n_hess; c->dust_mode = cfg->dust_mode;
+    c->P = (int64_t)cfg->n_im * cfg->n_im; c->hess_bins = bins;
+    c->like_floor = cfg->like_floor; c->dust_frac = cfg->dust_frac; c->mdf_cut = cfg->mdf_cut;
+    for (int b = 0; b < B; ++b) {
+        c->zp[b] = cfg->zp[b]; c->dust_coef[b] = cfg->dust_coef[b]; c->sky[b] = cfg->sky[b];
+        c->read_sigma[b] = cfg->read_sigma[b];
+    }
+    for (int h = 0; h < cfg->n_hess; ++h) c->hess[h] = cfg->hess[h];
+    int dev = 0, rc = PCMD_OK;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, dev);
+    c->h_imf_w = (double *)malloc((size_t)J * sizeof(double));
+    if (!c->h_imf_w) { delete c; return PCMD_ENOMEM; }
+    memcpy(c->h_imf_w, cfg->imf_w, (size_t)J * sizeof(double));
+#define TRY(x) do { rc = (x); if (rc) { pcmd_destroy(c); return rc; } } while (0)
+    TRY(upload(c, &c->d_age_idx, cfg->age_idx, (size_t)J));
+    TRY(upload(c, &c->d_feh_idx, cfg->feh_idx, (size_t)J));
+    TRY(upload(c, &c->d_imf_w, cfg->imf_w, (size_t)J));
+    TRY(upload(c, &c->d_absmag, cfg->absmag, (size_t)J * B));
+    TRY(upload(c, &c->d_feh_grid, cfg->feh_grid, (size_t)cfg->n_feh));
+    {   // PSF: kept as [B][K][K]; a separable PSF is expanded (column factor (x) row factor)
+        float *p2 = (float *)malloc((size_t)B * K * K * sizeof(float));
+        if (!p2) { pcmd_destroy(c); return PCMD_ENOMEM; }
+        for (int b = 0; b < B; ++b)
+            for (int y = 0; y < K; ++y)
+                for (int x = 0; x < K; ++x)
+                    p2[((size_t)b * K + y) * K + x] = cfg->psf_separable
+                        ? (float)((double)cfg->psf[((size_t)b * 2 + 1) * K + y] * (double)cfg->psf[((size_t)b * 2) * K + x])
+                        : cfg->psf[((size_t)b * K + y) * K + x];
+        rc = upload(c, &c->d_psf, p2, (size_t)B * K * K);
+        free(p2);
+        if (rc) { pcmd_destroy(c); return rc; }
+    }
+    {
+        uint64_t *mult = (uint64_t *)malloc((size_t)c->Jpad * sizeof(uint64_t));
+        if (!mult) { pcmd_destroy(c); return PCMD_ENOMEM; }
+        for (int j = 0; j < c->Jpad; ++j) mult[j] = splitmix64_host((uint64_t)j) | 1ull;
+        rc = upload(c, &c->d_mult, mult, (size_t)c->Jpad);
+        free(mult);
+        if (rc) { pcmd_destroy(c); return rc; }
+    }
+    {
+        DevHess dh[PCMD_MAX_HESS];
+        int64_t off = 0;
+        for (int h = 0; h < cfg->n_hess; ++h) {
+            const pcmd_hess_spec &s = cfg->hess[h];
+            dh[h].band_plus = s.band_plus; dh[h].band_minus = s.band_minus; dh[h].band_y = s.band_y;
+            dh[h].nx = s.nx; dh[h].ny = s.ny; dh[h].x_lo = (float)s.x_lo; dh[h].y_lo = (float)s.y_lo;
+            dh[h].inv_dx = (float)((double)s.nx / (s.x_hi - s.x_lo));
+            dh[h].inv_dy = (float)((double)s.ny / (s.y_hi - s.y_lo));
+            dh[h].bin_off = off; off += (int64_t)s.nx * s.ny;
+        }
+        TRY(upload(c, &c->d_hess_spec, dh, (size_t)cfg->n_hess));
+    }
+    {
+        cudaError_t e = cudaMalloc(&c->d_status, sizeof(int32_t));
+        if (e == cudaSuccess) e = cudaMemset(c->d_status, 0, sizeof(int32_t));
+        if (e != cudaSuccess) { c->last_cuda = (int)e; pcmd_destroy(c); return PCMD_ECUDA; }
+    }
+    TRY(pcmd_build_sky_tables(c));
+#undef TRY
+    cudaDeviceSynchronize();
+    *out = c;
+    return PCMD_OK;
+}
+
+extern "C" void pcmd_destroy(pcmd_ctx *c) {
+    if (!c) return;
+    cudaDeviceSynchronize();
+    free_scratch(c);
+    cudaFree(c->d_age_idx); cudaFree(c->d_feh_idx); cudaFree(c->d_imf_w); cudaFree(c->d_absmag);
+    cudaFree(c->d_feh_grid); cudaFree(c->d_psf); cudaFree(c->d_mult); cudaFree(c->d_hess_spec);
+    cudaFree(c->d_sky_tab); cudaFree(c->d_status); cudaFree(c->d_part);
+    cudaFree(c->d_mag); cudaFree(c->d_hessbuf); cudaFree(c->d_statbuf); cudaFree(c->d_lnl);
+    cudaFree(c->d_hess_data); cudaFree(c->d_data_stats);
+    if (c->h_pin) cudaFreeHost(c->h_pin);
+    if (c->stage_ev_valid) cudaEventDestroy(c->stage_ev);
+    free(c->h_imf_w);
+    delete c;
+}
+
+// ---------------------------------------------------------------------------------------------
+
+
+static int stage_params(pcmd_ctx *c, const pcmd_params *params, int n_models, cudaStream_t s) {
+    // upper bound of the raw sampler-table size of one model (sizing only, no method arithmetic):
+    // lambda_j <= max_a sfh_a * imf_w_j, and a table spans fewer than 20 sqrt(lambda) + 96 counts.
+    int64_t cap = 0;
+    for (int i = 0; i < n_models; ++i) {
+        const pcmd_params &p = params[i];
+        if (!p.sfh || !(p.feh_sigma > 0.0) || !isfinite(p.feh_mean) || !isfinite(p.feh_sigma) ||
+            !isfinite(p.dmod) || !(p.dust_med >= 0.0) || !isfinite(p.dust_med) || !(p.dust_sigma >= 0.0) ||
+            !isfinite(p.dust_sigma))
+            return PCMD_EINVAL;
+        double smax = 0.0;
+        for (int a = 0; a < c->A; ++a) {
+            if (!(p.sfh[a] >= 0.0) || !isfinite(p.sfh[a])) return PCMD_EINVAL;
+            if (p.sfh[a] > smax) smax = p.sfh[a];
+        }
+        double tot = 0.0;
+        for (int j = 0; j < c->J; ++j) {
+            const double lb = smax * c->h_imf_w[j];
+            if (lb > PCMD_LAMBDA_MAX) {
+                // the bound may be loose (MDF weight < 1); the kernel raises ERANGE on the true value
+                tot += 20.0 * 2048.0 + 96.0;
+            } else tot += 20.0 * sqrt(lb) + 96.0;
+        }
+        if ((int64_t)tot > cap) cap = (int64_t)tot;
+    }
+    if (cap > 0xFFFFFFF0ll) return PCMD_ERANGE;
+    int rc = ensure_scratch(c, n_models, cap);
+    if (rc) return rc;
+    double *hs = c->h_stage;
+    DevModel *hm = reinterpret_cast<DevModel *>(hs + (size_t)n_models * c->A);
+    for (int i = 0; i < n_models; ++i) {
+        memcpy(hs + (size_t)i * c->A, params[i].sfh, c->A * sizeof(double));
+        hm[i].feh_mean = params[i].feh_mean; hm[i].feh_sigma = params[i].feh_sigma;
+        hm[i].dmod = params[i].dmod; hm[i].dust_med = params[i].dust_med; hm[i].dust_sigma = params[i].dust_sigma;
+    }
+    PCMD_CUDA(c, cudaMemcpyAsync(c->d_sfh, hs, (size_t)n_models * c->A * sizeof(double), cudaMemcpyHostToDevice, s));
+    PCMD_CUDA(c, cudaMemcpyAsync(c->d_model, hm, (size_t)n_models * sizeof(DevModel), cudaMemcpyHostToDevice, s));
+    return PCMD_OK;
+}
+
+extern "C" int pcmd_simulate(pcmd_ctx *c, const pcmd_params *params, int32_t n_models, uint64_t seed,
+                             uint32_t model_index0, float *d_mag, float *d_flux_raw,
+                             uint64_t *d_count_hash, uint32_t *d_count_total, void *cuda_stream) {
+    if (!c || !params || n_models < 1 || !d_mag) return PCMD_EINVAL;
+    if ((d_count_hash == nullptr) != (d_count_total == nullptr)) return PCMD_EINVAL;
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    // the pinned staging buffer is reused: wait until the previous call's copies have run
+    if (c->stage_ev_valid) PCMD_CUDA(c, cudaEventSynchronize(c->stage_ev));
+    int rc = stage_params(c, params, n_models, s);
+    if (rc) return rc;
+    if (!c->stage_ev_valid) {
+        PCMD_CUDA(c, cudaEventCreateWithFlags(&c->stage_ev, cudaEventDisableTiming));
+        c->stage_ev_valid = 1;
+    }
+    PCMD_CUDA(c, cudaEventRecord(c->stage_ev, s));
+    PCMD_CUDA(c, cudaMemsetAsync(c->d_status, 0, sizeof(int32_t), s));
+    c->last_models = n_models;
+    if ((rc = pcmd_launch_stage1(c, n_models, s))) return rc;
+    if ((rc = pcmd_launch_stage2(c, n_models, seed, model_index0, d_flux_raw, d_count_hash, d_count_total, s))) return rc;
+    if (c->tap_dust)
+        PCMD_CUDA(c, cudaMemcpyAsync(c->tap_dust, c->d_fdust, (size_t)n_models * c->B * c->P * sizeof(float),
+                                     cudaMemcpyDeviceToDevice, s));
+    return pcmd_launch_conv_noise(c, n_models, seed, model_index0, d_mag, s);
+}
+
+extern "C" int pcmd_hess(pcmd_ctx *c, const float *d_mag, int32_t n_models, uint32_t *d_hess,
+                         pcmd_hess_stats *d_stats, void *cuda_stream) {
+    if (!c || !d_mag || !d_hess || n_models < 1 || c->n_hess < 1) return PCMD_EINVAL;
+    return pcmd_launch_hess(c, d_mag, n_models, d_hess, d_stats, (cudaStream_t)cuda_stream);
+}
+
+extern "C" int pcmd_loglike(pcmd_ctx *c, const uint32_t *d_hess_model, const pcmd_hess_stats *d_stats,
+                            int32_t n_models, const uint32_t *d_hess_data,
+                            const pcmd_hess_stats *d_data_stats, int32_t like_mode, double *d_loglike,
+                            void *cuda_stream) {
+    if (!c || !d_hess_model || !d_hess_data || !d_loglike || n_models < 1 || c->n_hess < 1) return PCMD_EINVAL;
+    if (like_mode < PCMD_LIKE_POISSON || like_mode > PCMD_LIKE_GAUSS_LITERAL) return PCMD_EINVAL;
+    if (like_mode != PCMD_LIKE_POISSON && (!d_stats || !d_data_stats)) return PCMD_EINVAL;
+    return pcmd_launch_loglike(c, d_hess_model, d_stats, n_models, d_hess_data, d_data_stats, like_mode,
+                               d_loglike, (cudaStream_t)cuda_stream);
+}
+
+extern "C" int64_t pcmd_hess_bins_total(const pcmd_ctx *c) { return c ? c->hess_bins : 0; }
+
+extern "C" int pcmd_evaluate_host(pcmd_ctx *c, const pcmd_params *params, int32_t n_models, uint64_t seed,
+                                  uint32_t model_index0, const uint32_t *h_hess_data,
+                                  const pcmd_hess_stats *h_data_stats, int32_t like_mode, double *h_loglike,
+                                  uint32_t *h_hess_out, pcmd_hess_stats *h_stats_out, void *cuda_stream) {
+    if (!c || !params || n_models < 1 || !h_hess_data || !h_loglike || c->n_hess < 1) return PCMD_EINVAL;
+    if (like_mode != PCMD_LIKE_POISSON && !h_data_stats) return PCMD_EINVAL;
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    const size_t hb = (size_t)c->hess_bins, nh = (size_t)c->n_hess;
+    if (n_models > c->eval_cap) {
+        cudaDeviceSynchronize();
+        cudaFree(c->d_mag); cudaFree(c->d_hessbuf); cudaFree(c->d_statbuf); cudaFree(c->d_lnl);
+        cudaFree(c->d_hess_data); cudaFree(c->d_data_stats);
+        if (c->h_pin) cudaFreeHost(c->h_pin);
+        c->d_mag = nullptr; c->d_hessbuf = nullptr; c->d_statbuf = nullptr; c->d_lnl = nullptr;
+        c->d_hess_data = nullptr; c->d_data_stats = nullptr; c->h_pin = nullptr; c->eval_cap = 0;
+        PCMD_CUDA(c, cudaMalloc(&c->d_mag, (size_t)n_models * c->B * c->P * sizeof(float)));
+        PCMD_CUDA(c, cudaMalloc(&c->d_hessbuf, (size_t)n_models * hb * sizeof(uint32_t)));
+        PCMD_CUDA(c, cudaMalloc(&c->d_statbuf, (size_t)n_models * nh * sizeof(pcmd_hess_stats)));
+        PCMD_CUDA(c, cudaMalloc(&c->d_lnl, (size_t)n_models * sizeof(double)));
+        PCMD_CUDA(c, cudaMalloc(&c->d_hess_data, hb * sizeof(uint32_t)));
+        PCMD_CUDA(c, cudaMalloc(&c->d_data_stats, nh * sizeof(pcmd_hess_stats)));
+        c->h_pin_bytes = hb * sizeof(uint32_t) + nh * sizeof(pcmd_hess_stats) +
+                         (size_t)n_models * (hb * sizeof(uint32_t) + nh * sizeof(pcmd_hess_stats) + sizeof(double));
+        PCMD_CUDA(c, cudaMallocHost(&c->h_pin, c->h_pin_bytes));
+        c->eval_cap = n_models;
+    }
+    // pinned layout: [data hess][data stats][model hess][model stats][lnl]
+    char *pin = (char *)c->h_pin;
+    uint32_t *p_dh = (uint32_t *)pin; pin += hb * sizeof(uint32_t);
+    pcmd_hess_stats *p_ds = (pcmd_hess_stats *)pin; pin += nh * sizeof(pcmd_hess_stats);
+    uint32_t *p_mh = (uint32_t *)pin; pin += (size_t)n_models * hb * sizeof(uint32_t);
+    pcmd_hess_stats *p_ms = (pcmd_hess_stats *)pin; pin += (size_t)n_models * nh * sizeof(pcmd_hess_stats);
+    double *p_l = (double *)pin;
+    memcpy(p_dh, h_hess_data, hb * sizeof(uint32_t));
+    PCMD_CUDA(c, cudaMemcpyAsync(c->d_hess_data, p_dh, hb * sizeof(uint32_t), cudaMemcpyHostToDevice, s));
+    if (h_data_stats) {
+        memcpy(p_ds, h_data_stats, nh * sizeof(pcmd_hess_stats));
+        PCMD_CUDA(c, cudaMemcpyAsync(c->d_data_stats, p_ds, nh * sizeof(pcmd_hess_stats), cudaMemcpyHostToDevice, s));
+    }
+    int rc = pcmd_simulate(c, params, n_models, seed, model_index0, c->d_mag, nullptr, nullptr, nullptr, cuda_stream);
+    if (rc) return rc;
+    if ((rc = pcmd_launch_hess(c, c->d_mag, n_models, c->d_hessbuf, c->d_statbuf, s))) return rc;
+    if ((rc = pcmd_launch_loglike(c, c->d_hessbuf, c->d_statbuf, n_models, c->d_hess_data,
+                                  h_data_stats ? c->d_data_stats : nullptr, like_mode, c->d_lnl, s)))
+        return rc;
+    PCMD_CUDA(c, cudaMemcpyAsync(p_l, c->d_lnl, (size_t)n_models * sizeof(double), cudaMemcpyDeviceToHost, s));
+    if (h_hess_out)
+        PCMD_CUDA(c, cudaMemcpyAsync(p_mh, c->d_hessbuf, (size_t)n_models * hb * sizeof(uint32_t), cudaMemcpyDeviceToHost, s));
+    if (h_stats_out)
+        PCMD_CUDA(c, cudaMemcpyAsync(p_ms, c->d_statbuf, (size_t)n_models * nh * sizeof(pcmd_hess_stats), cudaMemcpyDeviceToHost, s));
+    int32_t st = 0;
+    PCMD_CUDA(c, cudaMemcpyAsync(&st, c->d_status, sizeof(int32_t), cudaMemcpyDeviceToHost, s));
+    PCMD_CUDA(c, cudaStreamSynchronize(s));
+    memcpy(h_loglike, p_l, (size_t)n_models * sizeof(double));
+    if (h_hess_out) memcpy(h_hess_out, p_mh, (size_t)n_models * hb * sizeof(uint32_t));
+    if (h_stats_out) memcpy(h_stats_out, p_ms, (size_t)n_models * nh * sizeof(pcmd_hess_stats));
+    return st;
+}
+
+// ---------------------------------------------------------------------------------------------
+extern "C" int pcmd_debug_weights(pcmd_ctx *c, int32_t model, double *h_lambda, float *h_flux, uint32_t *h_k0,
+                                  uint32_t *h_len, uint32_t *h_tables, int64_t cap, int64_t *n_tables) {
+    if (!c || model < 0 || model >= c->last_models) return PCMD_EINVAL;
+    PCMD_CUDA(c, cudaDeviceSynchronize());
+    const int J = c->J;
+    if (h_lambda)
+        PCMD_CUDA(c, cudaMemcpy(h_lambda, c->d_lambda + (size_t)model * J, (size_t)J * sizeof(double), cudaMemcpyDeviceToHost));
+    PointRec *rec = (PointRec *)malloc((size_t)J * sizeof(PointRec));
+    if (!rec) return PCMD_ENOMEM;
+    cudaError_t e = cudaMemcpy(rec, c->d_rec + (size_t)model * c->Jpad, (size_t)J * sizeof(PointRec), cudaMemcpyDeviceToHost);
+    if (e != cudaSuccess) { free(rec); c->last_cuda = (int)e; return PCMD_ECUDA; }
+    int64_t total = 0;
+    for (int j = 0; j < J; ++j) {
+        if (h_k0) h_k0[j] = rec[j].k0;
+        if (h_len) h_len[j] = rec[j].len;
+        if (h_flux) for (int b = 0; b < c->B; ++b) h_flux[(size_t)j * c->B + b] = rec[j].f[b];
+        total += rec[j].len;   // tables are compact and in point order
+    }
+    free(rec);
+    if (n_tables) *n_tables = total;
+    if (h_tables) {
+        int64_t n = total < cap ? total : cap;
+        uint32_t *tmp = (uint32_t *)malloc((size_t)(n ? n : 1) * sizeof(uint32_t));
+        if (!tmp) return PCMD_ENOMEM;
+        e = cudaMemcpy(tmp, c->d_tab + (size_t)model * c->cap_raw, (size_t)n * sizeof(uint32_t), cudaMemcpyDeviceToHost);
+        if (e != cudaSuccess) { free(tmp); c->last_cuda = (int)e; return PCMD_ECUDA; }
+        for (int64_t i = 0; i < n; ++i) h_tables[i] = tmp[i] + 1u;  // stored minus 1 on the device
+        free(tmp);
+    }
+    return PCMD_OK;
+}
+
+extern "C" int pcmd_debug_taps(pcmd_ctx *c, float *d_flux_dust, float *d_flux_conv) {
+    if (!c) return PCMD_EINVAL;
+    c->tap_dust = d_flux_dust; c->tap_conv = d_flux_conv;
+    return PCMD_OK;
+}
+
+__global__ void k_debug_philox(uint32_t k0, uint32_t k1, const uint32_t *__restrict__ ctr, int64_t n,
+                               uint32_t *__restrict__ out) {
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    uint32_t w[4];
+    philox4x32_10(k0, k1, ctr[4 * i], ctr[4 * i + 1], ctr[4 * i + 2], ctr[4 * i + 3], w);
+    out[4 * i] = w[0]; out[4 * i + 1] = w[1]; out[4 * i + 2] = w[2]; out[4 * i + 3] = w[3];
+}
+
+extern "C" int pcmd_debug_philox(uint64_t seed, const uint32_t *h_ctr, int64_t n, uint32_t *h_out) {
+    if (!h_ctr || !h_out || n < 1) return PCMD_EINVAL;
+    uint32_t *d_c = nullptr, *d_o = nullptr;
+    pcmd_ctx *none = nullptr;
+    PCMD_CUDA(none, cudaMalloc(&d_c, (size_t)n * 16));
+    PCMD_CUDA(none, cudaMalloc(&d_o, (size_t)n * 16));
+    PCMD_CUDA(none, cudaMemcpy(d_c, h_ctr, (size_t)n * 16, cudaMemcpyHostToDevice));
+    k_debug_philox<<<(unsigned)((n + 127) / 128), 128>>>((uint32_t)(seed & 0xFFFFFFFFull), (uint32_t)(seed >> 32), d_c, n, d_o);
+    PCMD_CUDA(none, cudaGetLastError());
+    PCMD_CUDA(none, cudaMemcpy(h_out, d_o, (size_t)n * 16, cudaMemcpyDeviceToHost));
+    cudaFree(d_c); cudaFree(d_o);
+    return PCMD_OK;
+}
+
+extern "C" int pcmd_status(pcmd_ctx *c, void *cuda_stream) {
+    if (!c) return PCMD_EINVAL;
+    PCMD_CUDA(c, cudaStreamSynchronize((cudaStream_t)cuda_stream));
+    int32_t st = 0;
+    PCMD_CUDA(c, cudaMemcpy(&st, c->d_status, sizeof(int32_t), cudaMemcpyDeviceToHost));
+    return st;
+}
+
+extern "C" int pcmd_last_cuda_error(const pcmd_ctx *c) { return c ? c->last_cuda : 0; }
+extern "C" int64_t pcmd_launch_count(const pcmd_ctx *c) { return c ? c->launches : 0; }
+
+extern "C" int pcmd_set_option(pcmd_ctx *c, const char *name, int64_t value) {
+    if (!c || !name) return PCMD_EINVAL;
+    if (strcmp(name, "stage2") == 0) { int64_t old = c->opt_stage2; c->opt_stage2 = value; return (int)old; }
+    return PCMD_EINVAL;
+}

@@ -1,0 +1,115 @@
+// conv_noise.cu -- stage 4: per-band PSF convolution with circular boundary (
+// R-Q9), and stage 5 fused into its epilogue: sky, shot/read noise, magnitudes (PAPER.md:83,
+// 127-128,178; R-Q11).  Shared-memory tiled direct 2-D convolution (works for any PSF).
+#include "pcmd_internal.cuh"
+
+#define CV_TX 32
+#define CV_TY 32
+#define CV_ROWS 8   // blockDim.y; each thread computes CV_TY / CV_ROWS outputs
+
+struct CvArgs {
+    const float *F;      // [n_models][B][P] dusty flux
+    const float *psf;    // [B][K][K]
+    float *mag;          // [n_models][B][P]
+    float *tap_conv;     // optional
+    const uint32_t *sky_tab;
+    PointRec sky_rec[4];
+    int N, B, K;
+    int64_t P;
+    int shot_noise, poisson_sky;
+    uint32_t key0, key1, model0;
+    double zp[4], sky[4], read_sigma[4];
+};
+
+__global__ void __launch_bounds__(CV_TX * CV_ROWS) k_conv_noise(const CvArgs a) {
+    extern __shared__ float sm[];
+    const int K = a.K, r = (K - 1) / 2, N = a.N;
+    const int TW = CV_TX + K - 1, TH = CV_TY + K - 1;
+    float *tile = sm;              // [TH][TW]
+    float *spsf = sm + TH * TW;    // [K][K]
+    const int mb = blockIdx.z, m = mb / a.B, b = mb - m * a.B;
+    const float *F = a.F + (size_t)mb * a.P;
+    const int x0 = blockIdx.x * CV_TX, y0 = blockIdx.y * CV_TY;
+    const int tid = threadIdx.y * CV_TX + threadIdx.x, nt = CV_TX * CV_ROWS;
+    for (int t = tid; t < K * K; t += nt) spsf[t] = a.psf[(size_t)b * K * K + t];
+    for (int t = tid; t < TH * TW; t += nt) {
+        int i = t / TW, j = t - i * TW;
+        int yy = (y0 - r + i) % N; if (yy < 0) yy += N;
+        int xx = (x0 - r + j) % N; if (xx < 0) xx += N;
+        tile[t] = F[(size_t)yy * N + xx];
+    }
+    __syncthreads();
+    const int lx = threadIdx.x;
+    float acc[CV_TY / CV_ROWS];
+#pragma unroll
+    for (int q = 0; q < CV_TY / CV_ROWS; ++q) acc[q] = 0.f;
+    for (int ka = 0; ka < K; ++ka)
+        for (int kb = 0; kb < K; ++kb) {
+            const float w = spsf[ka * K + kb];
+#pragma unroll
+            for (int q = 0; q < CV_TY / CV_ROWS; ++q) {
+                const int ly = threadIdx.y + q * CV_ROWS;
+                acc[q] = fmaf(w, tile[(ly + 2 * r - ka) * TW + (lx + 2 * r - kb)], acc[q]);
+            }
+        }
+    const int x = x0 + lx;
+    if (x >= N) return;
+    const uint32_t mctr = a.model0 + (uint32_t)m;
+    const double sky = a.sky[b], rs = a.read_sigma[b], zp = a.zp[b];
+    const bool psky = a.poisson_sky && sky > 0.0;
+    const bool need_g = a.shot_noise || rs > 0.0;
+#pragma unroll
+    for (int q = 0; q < CV_TY / CV_ROWS; ++q) {
+        const int y = y0 + threadIdx.y + q * CV_ROWS;
+        if (y >= N) continue;
+        const uint32_t p = (uint32_t)y * (uint32_t)N + (uint32_t)x;
+        const size_t o = (size_t)mb * a.P + p;
+        if (a.tap_conv) a.tap_conv[o] = acc[q];
+        const double Gi = (double)acc[q];
+        uint32_t w[4];
+        double g = 0.0;
+        if (need_g) {
+            philox4x32_10(a.key0, a.key1, p, (uint32_t)b, mctr, 2u, w);
+            g = normal_from_words(w[0], w[1]);
+        }
+        double Cp;
+        if (psky) {
+            philox4x32_10(a.key0, a.key1, p, (uint32_t)b, mctr, 3u, w);
+            const PointRec sr = a.sky_rec[b];
+            double Kc = (double)(sr.k0 + count_below(a.sky_tab + sr.off, sr.len, w[0]));
+            double var = (a.shot_noise ? fmax(Gi, 0.0) : 0.0) + rs * rs;
+            Cp = Gi + Kc + sqrt(var) * g;
+        } else {
+            double C = Gi + sky;
+            double var = (a.shot_noise ? fmax(C, 0.0) : 0.0) + rs * rs;
+            Cp = C + sqrt(var) * g;
+        }
+        double arg = Cp - sky;
+        a.mag[o] = (arg > 0.0) ? (float)(zp - 2.5 * log10(arg)) : __int_as_float(0x7fc00000);
+    }
+}
+
+int pcmd_launch_conv_noise(pcmd_ctx *c, int n_models, uint64_t seed, uint32_t model0, float *d_mag,
+                           cudaStream_t s) {
+    CvArgs a;
+    a.F = c->d_fdust; a.psf = c->d_psf; a.mag = d_mag; a.tap_conv = c->tap_conv;
+    a.sky_tab = c->d_sky_tab;
+    for (int b = 0; b < 4; ++b) {
+        a.sky_rec[b] = c->sky_rec[b];
+        a.zp[b] = c->zp[b]; a.sky[b] = c->sky[b]; a.read_sigma[b] = c->read_sigma[b];
+    }
+    a.N = c->N; a.B = c->B; a.K = c->K; a.P = c->P;
+    a.shot_noise = c->shot_noise; a.poisson_sky = c->poisson_sky;
+    a.key0 = (uint32_t)(seed & 0xFFFFFFFFull); a.key1 = (uint32_t)(seed >> 32); a.model0 = model0;
+    const int K = c->K;
+    size_t smem = ((size_t)(CV_TX + K - 1) * (CV_TY + K - 1) + (size_t)K * K) * sizeof(float);
+    static size_t smem_set = 0;
+    if (smem > 48 * 1024 && smem > smem_set) {
+        PCMD_CUDA(c, cudaFuncSetAttribute(k_conv_noise, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        smem_set = smem;
+    }
+    dim3 grid((c->N + CV_TX - 1) / CV_TX, (c->N + CV_TY - 1) / CV_TY, n_models * c->B);
+    k_conv_noise<<<grid, dim3(CV_TX, CV_ROWS), smem, s>>>(a);
+    PCMD_LAUNCHED(c);
+    return PCMD_OK;
+}

@@ -1,0 +1,199 @@
+// hess_like.cu -- stage 6: Hess diagram = 2-D histogram of (colour, magnitude) (PAPER.md:57,130,
+// 218; R-Q13) with a block-private shared-memory histogram, and stage 7: Poisson log-likelihood
+// (north_star; R-Q15) and the paper's Eq. 2-4 (R-Q14).
+#include "pcmd_internal.cuh"
+
+#define HS_THREADS 256
+#define HS_PIX_PER_BLOCK 4096
+
+// Binning arithmetic, fp32, no contraction:
+// x = fl(mp - mm); t = fl(fl(x - x_lo) * inv_dx); ix = floor(t); half-open.
+template <bool SMEM>
+__global__ void __launch_bounds__(HS_THREADS) k_hess(const float *__restrict__ mag, int B, int64_t P,
+                                                     const DevHess *__restrict__ specs, int n_hess,
+                                                     int64_t bins_total, uint32_t *__restrict__ hess,
+                                                     pcmd_hess_stats *__restrict__ part) {
+    extern __shared__ uint32_t sh[];
+    const int h = blockIdx.y, m = blockIdx.z;
+    const DevHess S = specs[h];
+    const int nbins = S.nx * S.ny;
+    uint32_t *gh = hess + (size_t)m * bins_total + S.bin_off;
+    if (SMEM) {
+        for (int t = threadIdx.x; t < nbins; t += HS_THREADS) sh[t] = 0;
+        __syncthreads();
+    }
+    const float *mp = mag + ((size_t)m * B + S.band_plus) * P;
+    const float *mm = mag + ((size_t)m * B + S.band_minus) * P;
+    const float *my = mag + ((size_t)m * B + S.band_y) * P;
+    uint32_t n_in = 0, n_out = 0, n_bad = 0;
+    double sx = 0.0, sy = 0.0;
+    const int64_t p0 = (int64_t)blockIdx.x * HS_PIX_PER_BLOCK;
+    const int64_t p1 = min(P, p0 + HS_PIX_PER_BLOCK);
+    for (int64_t p = p0 + threadIdx.x; p < p1; p += HS_THREADS) {
+        const float a = mp[p], b = mm[p], y = my[p];
+        if (isnan(a) || isnan(b) || isnan(y)) { n_bad++; continue; }
+        const float x = __fsub_rn(a, b);
+        const float fx = floorf(__fmul_rn(__fsub_rn(x, S.x_lo), S.inv_dx));
+        const float fy = floorf(__fmul_rn(__fsub_rn(y, S.y_lo), S.inv_dy));
+        if (!(fx >= 0.0f) || !(fx < (float)S.nx) || !(fy >= 0.0f) || !(fy < (float)S.ny)) { n_out++; continue; }
+        const int bin = (int)fy * S.nx + (int)fx;
+        if (SMEM) atomicAdd(&sh[bin], 1u); else atomicAdd(&gh[bin], 1u);
+        n_in++; sx += (double)x; sy += (double)y;
+    }
+    // block reduction of the stats in a fixed order (deterministic)
+    __shared__ double r_sx[HS_THREADS / 32], r_sy[HS_THREADS / 32];
+    __shared__ uint32_t r_n[3][HS_THREADS / 32];
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) {
+        n_in += __shfl_down_sync(0xffffffffu, n_in, d);
+        n_out += __shfl_down_sync(0xffffffffu, n_out, d);
+        n_bad += __shfl_down_sync(0xffffffffu, n_bad, d);
+        sx += __shfl_down_sync(0xffffffffu, sx, d);
+        sy += __shfl_down_sync(0xffffffffu, sy, d);
+    }
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    if (lane == 0) { r_n[0][wid] = n_in; r_n[1][wid] = n_out; r_n[2][wid] = n_bad; r_sx[wid] = sx; r_sy[wid] = sy; }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        pcmd_hess_stats st = {0, 0, 0, 0, 0.0, 0.0};
+        for (int w = 0; w < HS_THREADS / 32; ++w) {
+            st.n_in += r_n[0][w]; st.n_out += r_n[1][w]; st.n_bad += r_n[2][w];
+            st.sum_x += r_sx[w]; st.sum_y += r_sy[w];
+        }
+        part[((size_t)m * n_hess + h) * gridDim.x + blockIdx.x] = st;
+    }
+    if (SMEM) {
+        for (int t = threadIdx.x; t < nbins; t += HS_THREADS) {
+            uint32_t v = sh[t];
+            if (v) atomicAdd(&gh[t], v);
+        }
+    }
+}
+
+__global__ void k_hess_stats(const pcmd_hess_stats *__restrict__ part, int nblk,
+                             pcmd_hess_stats *__restrict__ out) {
+    // one thread per (model, hess): partials added in block order
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= (int)gridDim.y) { /* unused */ }
+    pcmd_hess_stats st = {0, 0, 0, 0, 0.0, 0.0};
+    const pcmd_hess_stats *p = part + (size_t)blockIdx.x * nblk;
+    if (threadIdx.x == 0) {
+        for (int b = 0; b < nblk; ++b) {
+            st.n_in += p[b].n_in; st.n_out += p[b].n_out; st.n_bad += p[b].n_bad;
+            st.sum_x += p[b].sum_x; st.sum_y += p[b].sum_y;
+        }
+        out[blockIdx.x] = st;
+    }
+}
+
+int pcmd_launch_hess(pcmd_ctx *c, const float *d_mag, int n_models, uint32_t *d_hess,
+                     pcmd_hess_stats *d_stats, cudaStream_t s) {
+    const int nblk = (int)((c->P + HS_PIX_PER_BLOCK - 1) / HS_PIX_PER_BLOCK);
+    const int64_t need = (int64_t)n_models * c->n_hess * nblk;
+    if (need > c->part_cap) {
+        if (c->d_part) cudaFree(c->d_part);
+        c->d_part = nullptr; c->part_cap = 0;
+        PCMD_CUDA(c, cudaMalloc(&c->d_part, need * sizeof(pcmd_hess_stats)));
+        c->part_cap = need;
+    }
+    PCMD_CUDA(c, cudaMemsetAsync(d_hess, 0, (size_t)n_models * c->hess_bins * sizeof(uint32_t), s));
+    int maxbins = 0;
+    for (int h = 0; h < c->n_hess; ++h) maxbins = max(maxbins, c->hess[h].nx * c->hess[h].ny);
+    size_t smem = (size_t)maxbins * sizeof(uint32_t);
+    dim3 grid(nblk, c->n_hess, n_models);
+    if (smem <= 200 * 1024) {
+        static size_t smem_set = 0;
+        if (smem > 48 * 1024 && smem > smem_set) {
+            PCMD_CUDA(c, cudaFuncSetAttribute(k_hess<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+            smem_set = smem;
+        }
+        k_hess<true><<<grid, HS_THREADS, smem, s>>>(d_mag, c->B, c->P, c->d_hess_spec, c->n_hess,
+                                                    c->hess_bins, d_hess, c->d_part);
+    } else {
+        k_hess<false><<<grid, HS_THREADS, 0, s>>>(d_mag, c->B, c->P, c->d_hess_spec, c->n_hess,
+                                                  c->hess_bins, d_hess, c->d_part);
+    }
+    PCMD_LAUNCHED(c);
+    if (d_stats) {
+        k_hess_stats<<<n_models * c->n_hess, 32, 0, s>>>(c->d_part, nblk, d_stats);
+        PCMD_LAUNCHED(c);
+    }
+    return PCMD_OK;
+}
+
+// ---------------------------------------------------------------------------------------------
+// Stage 7.  One block per model; every reduction is a fixed-order tree (deterministic).
+#define LL_THREADS 256
+
+__device__ double block_sum(double v, double *scratch) {
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) v += __shfl_down_sync(0xffffffffu, v, d);
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    __syncthreads();
+    if (lane == 0) scratch[wid] = v;
+    __syncthreads();
+    double t = 0.0;
+    for (int w = 0; w < LL_THREADS / 32; ++w) t += scratch[w];
+    return t;  // same value in every thread
+}
+
+__global__ void __launch_bounds__(LL_THREADS) k_loglike(const uint32_t *__restrict__ hm_all,
+                                                        const pcmd_hess_stats *__restrict__ sm_all,
+                                                        const uint32_t *__restrict__ hd_all,
+                                                        const pcmd_hess_stats *__restrict__ sd_all,
+                                                        const DevHess *__restrict__ specs, int n_hess,
+                                                        int64_t bins_total, int mode, double m_floor,
+                                                        double *__restrict__ out) {
+    __shared__ double scratch[LL_THREADS / 32];
+    const int m = blockIdx.x;
+    double total = 0.0;
+    for (int h = 0; h < n_hess; ++h) {
+        const DevHess S = specs[h];
+        const int nb = S.nx * S.ny;
+        const uint32_t *hm = hm_all + (size_t)m * bins_total + S.bin_off;
+        const uint32_t *hd = hd_all + S.bin_off;
+        double nd = 0.0, nm = 0.0;
+        for (int i = threadIdx.x; i < nb; i += LL_THREADS) { nd += (double)hd[i]; nm += (double)hm[i]; }
+        const double Nd = block_sum(nd, scratch), Nm = block_sum(nm, scratch);
+        if (!(Nm > 0.0) || !(Nd > 0.0)) { total = -INFINITY; continue; }
+        double L = 0.0;
+        if (mode == PCMD_LIKE_POISSON) {
+            const double sc = Nd / Nm;
+            for (int i = threadIdx.x; i < nb; i += LL_THREADS) {
+                const uint32_t d = hd[i], mo = hm[i];
+                if (d == 0 && mo == 0) continue;
+                const double mu = sc * fmax((double)mo, m_floor);
+                L += (double)d * log(mu) - mu - lgamma((double)d + 1.0);
+            }
+            L = block_sum(L, scratch);
+        } else {
+            for (int i = threadIdx.x; i < nb; i += LL_THREADS) {
+                const double d = (double)hd[i], mo = (double)hm[i];
+                const double diff = d / Nd - mo / Nm;
+                double var;
+                if (mode == PCMD_LIKE_GAUSS_LITERAL) { double sg = fmax(sqrt(d * d + mo * mo), 2.0); var = sg * sg; }
+                else {
+                    double ed = fmax(sqrt(d), 1.0) / Nd, em = fmax(sqrt(mo), 1.0) / Nm;
+                    var = ed * ed + em * em;
+                }
+                L += -(diff * diff) / (2.0 * var);
+            }
+            L = block_sum(L, scratch);
+            const pcmd_hess_stats a = sm_all[(size_t)m * n_hess + h], b = sd_all[h];
+            const double Cd = b.sum_x / (double)b.n_in, Cm = a.sum_x / (double)a.n_in;
+            const double Md = b.sum_y / (double)b.n_in, Mm = a.sum_y / (double)a.n_in;
+            L += -((Cd - Cm) * (Cd - Cm)) / (2.0 * 0.05 * 0.05) - ((Md - Mm) * (Md - Mm)) / (2.0 * 0.05 * 0.05);
+        }
+        total += L;
+    }
+    if (threadIdx.x == 0) out[m] = total;
+}
+
+int pcmd_launch_loglike(pcmd_ctx *c, const uint32_t *d_hm, const pcmd_hess_stats *d_sm, int n_models,
+                        const uint32_t *d_hd, const pcmd_hess_stats *d_sd, int mode, double *d_out,
+                        cudaStream_t s) {
+    k_loglike<<<n_models, LL_THREADS, 0, s>>>(d_hm, d_sm, d_hd, d_sd, c->d_hess_spec, c->n_hess,
+                                              c->hess_bins, mode, c->like_floor, d_out);
+    PCMD_LAUNCHED(c);
+    return PCMD_OK;
+}

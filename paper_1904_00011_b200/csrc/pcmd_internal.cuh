@@ -1,0 +1,140 @@
+// pcmd_internal.cuh -- shared declarations of the CUDA path (never included by oracle/).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include "../../include/pcmd.h"
+
+#define PCMD_LAMBDA_MAX 4194304.0 /* 2^22, R-C2 */
+
+// Per isochrone point record consumed by stage 2 (32 bytes, one group of 4 points = 128 B).
+struct __align__(16) PointRec {
+    uint32_t T0;    // first stored threshold minus 1 (draw > T0 <=> n > k0); 0xFFFFFFFF if none
+    uint32_t off;   // offset of the stored thresholds (minus 1 each) in the model's table
+    uint32_t len;   // number of stored thresholds
+    uint32_t k0;    // first count whose T > 0
+    float f[4];     // flux of one star in each band (electrons), unused bands 0
+};
+
+struct DevHess {
+    int32_t band_plus, band_minus, band_y, nx, ny;
+    float x_lo, y_lo, inv_dx, inv_dy;
+    int64_t bin_off;  // offset of this diagram inside a model's Hess block
+};
+
+struct DevModel {          // per-model scalars staged from pcmd_params
+    double feh_mean, feh_sigma, dmod, dust_med, dust_sigma;
+};
+
+struct pcmd_ctx {
+    // ---- configuration (host copies)
+    int32_t N, B, A, Z, J, Jpad, K, psf_sep, shot_noise, poisson_sky, n_hess, dust_mode;
+    int64_t P, hess_bins;
+    double like_floor, dust_frac, mdf_cut;
+    double zp[PCMD_MAX_BANDS], dust_coef[PCMD_MAX_BANDS], sky[PCMD_MAX_BANDS], read_sigma[PCMD_MAX_BANDS];
+    pcmd_hess_spec hess[PCMD_MAX_HESS];
+    double *h_imf_w;       // [J] host copy, used only to size scratch
+    // ---- device constants
+    int32_t *d_age_idx, *d_feh_idx;
+    double *d_imf_w, *d_absmag, *d_feh_grid;
+    float *d_psf;          // [B][K][K] or [B][2][K]
+    uint64_t *d_mult;      // [Jpad] splitmix64(j)|1
+    DevHess *d_hess_spec;  // [n_hess]
+    uint32_t *d_sky_tab;   // [B][sky_cap] stored thresholds minus 1 of Poisson(sky_b)
+    PointRec sky_rec[PCMD_MAX_BANDS]; uint32_t sky_cap;
+    // ---- per-call scratch, sized for cap_models
+    int32_t cap_models;
+    int64_t cap_raw;       // entries of raw table scratch per model
+    double *d_sfh;         // [cap_models][A]
+    DevModel *d_model;     // [cap_models]
+    double *h_stage;       // pinned staging for sfh + DevModel
+    size_t h_stage_bytes;
+    double *d_mdfw;        // [cap_models][Z]
+    double *d_lambda;      // [cap_models][J]
+    uint32_t *d_rawcnt;    // [cap_models][J+1] raw table range sizes -> exclusive offsets
+    uint32_t *d_klo;       // [cap_models][J]
+    double *d_q;           // [cap_models][cap_raw] pmf ratios, then thresholds (as uint64)
+    uint32_t *d_stcnt;     // [cap_models][J+1] stored counts -> exclusive offsets
+    uint32_t *d_tab;       // [cap_models][cap_raw] stored thresholds minus 1
+    PointRec *d_rec;       // [cap_models][Jpad]
+    float *d_fdust;        // [cap_models][B][P]
+    int32_t *d_status;     // device status word
+    // hess / loglike scratch
+    pcmd_hess_stats *d_part; int64_t part_cap;   // per-block partial stats
+    // evaluate_host scratch
+    float *d_mag; uint32_t *d_hessbuf; pcmd_hess_stats *d_statbuf; double *d_lnl;
+    uint32_t *d_hess_data; pcmd_hess_stats *d_data_stats;
+    int32_t eval_cap;
+    void *h_pin; size_t h_pin_bytes;
+    // taps / options / bookkeeping
+    float *tap_dust, *tap_conv;
+    int64_t opt_stage2;
+    int32_t last_models;
+    int last_cuda;
+    int64_t launches;
+    int sm_count;
+    cudaEvent_t stage_ev; int stage_ev_valid;
+};
+
+// error helpers ---------------------------------------------------------------------------
+#define PCMD_CUDA(ctx, call)                                              \
+    do {                                                                  \
+        cudaError_t e__ = (call);                                         \
+        if (e__ != cudaSuccess) {                                         \
+            if (ctx) (ctx)->last_cuda = (int)e__;                         \
+            return (e__ == cudaErrorMemoryAllocation) ? PCMD_ENOMEM : PCMD_ECUDA; \
+        }                                                                 \
+    } while (0)
+#define PCMD_LAUNCHED(ctx)                                                \
+    do {                                                                  \
+        (ctx)->launches++;                                                \
+        cudaError_t e__ = cudaGetLastError();                             \
+        if (e__ != cudaSuccess) { (ctx)->last_cuda = (int)e__; return PCMD_ECUDA; } \
+    } while (0)
+
+// Philox4x32-10 (R-C1), device side ----------------------------------------------------------
+#define PHILOX_M0 0xD2511F53u
+#define PHILOX_M1 0xCD9E8D57u
+#define PHILOX_W0 0x9E3779B9u
+#define PHILOX_W1 0xBB67AE85u
+
+__device__ __forceinline__ void philox4x32_10(uint32_t k0, uint32_t k1, uint32_t c0, uint32_t c1,
+                                              uint32_t c2, uint32_t c3, uint32_t out[4]) {
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+        uint32_t h0 = __umulhi(PHILOX_M0, c0), l0 = PHILOX_M0 * c0;
+        uint32_t h1 = __umulhi(PHILOX_M1, c2), l1 = PHILOX_M1 * c2;
+        c0 = h1 ^ c1 ^ k0; c1 = l1; c2 = h0 ^ c3 ^ k1; c3 = l0;
+        k0 += PHILOX_W0; k1 += PHILOX_W1;
+    }
+    out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+
+// Box-Muller normal from two words (R-C4), fp64: it is O(P) work, not O(P J).
+__device__ __forceinline__ double normal_from_words(uint32_t w0, uint32_t w1) {
+    double u1 = ((double)w0 + 0.5) * (1.0 / 4294967296.0);
+    double u2 = ((double)w1 + 0.5) * (1.0 / 4294967296.0);
+    return sqrt(-2.0 * log(u1)) * cos(6.283185307179586476925 * u2);
+}
+
+// #{i < len : u > T[i]} for non-decreasing T (thresholds stored minus 1)
+__device__ __forceinline__ uint32_t count_below(const uint32_t *__restrict__ T, uint32_t len, uint32_t u) {
+    uint32_t lo = 0, hi = len;
+    while (lo < hi) {
+        uint32_t mid = (lo + hi) >> 1;
+        if (u > T[mid]) lo = mid + 1; else hi = mid;
+    }
+    return lo;
+}
+
+// launchers implemented in the stage files ---------------------------------------------------
+int pcmd_launch_stage1(pcmd_ctx *c, int n_models, cudaStream_t s);
+int pcmd_build_sky_tables(pcmd_ctx *c);
+int pcmd_launch_stage2(pcmd_ctx *c, int n_models, uint64_t seed, uint32_t model0, float *d_flux_raw,
+                       uint64_t *d_hash, uint32_t *d_total, cudaStream_t s);
+int pcmd_launch_conv_noise(pcmd_ctx *c, int n_models, uint64_t seed, uint32_t model0, float *d_mag,
+                           cudaStream_t s);
+int pcmd_launch_hess(pcmd_ctx *c, const float *d_mag, int n_models, uint32_t *d_hess,
+                     pcmd_hess_stats *d_stats, cudaStream_t s);
+int pcmd_launch_loglike(pcmd_ctx *c, const uint32_t *d_hm, const pcmd_hess_stats *d_sm, int n_models,
+                        const uint32_t *d_hd, const pcmd_hess_stats *d_sd, int mode, double *d_out,
+                        cudaStream_t s);

@@ -1,0 +1,250 @@
+// stage1.cu -- isochrone weighting and sampler tables (DESIGN.md R-C2,R-C3).
+// Everything that decides a star count is fp64 with explicit round-to-nearest intrinsics
+// (__dmul_rn etc. are never contracted into FMAs), so the tables are bit-identical on any
+// IEEE machine.
+#include "pcmd_internal.cuh"
+
+#define TWO_M64 5.42101086242752217e-20
+#define TWO32 4294967296.0
+
+// e^-t, t >= 0, from basic operations only (R-C3): degree-6 Taylor polynomial of e^-r at
+// r = t 2^-16 in Horner form, then sixteen squarings.
+__device__ double expneg_basic(double t) {
+    if (t > 64.0) return 0.0;
+    const double c[7] = {0.0, 1.0, 1.0 / 2.0, 1.0 / 3.0, 1.0 / 4.0, 1.0 / 5.0, 1.0 / 6.0};
+    double r = __dmul_rn(t, 1.0 / 65536.0);
+    double p = 1.0;
+#pragma unroll
+    for (int k = 6; k >= 1; --k) p = __dsub_rn(1.0, __dmul_rn(__dmul_rn(r, c[k]), p));
+#pragma unroll
+    for (int i = 0; i < 16; ++i) p = __dmul_rn(p, p);
+    return p;
+}
+
+// grid = n_models.  Thread 0 computes the MDF weights in the stated order; all threads then
+// compute lambda_j and the per-star fluxes.
+__global__ void k_weights(const DevModel *__restrict__ mdl, const double *__restrict__ sfh,
+                          const double *__restrict__ feh_grid, const int32_t *__restrict__ age_idx,
+                          const int32_t *__restrict__ feh_idx, const double *__restrict__ imf_w,
+                          const double *__restrict__ absmag, int A, int Z, int J, int Jpad, int B,
+                          double mdf_cut, double zp0, double zp1, double zp2, double zp3,
+                          double *__restrict__ mdfw_out, double *__restrict__ lambda_out,
+                          PointRec *__restrict__ rec_out, int32_t *status) {
+    extern __shared__ double w[];  // [Z]
+    const int m = blockIdx.x;
+    const DevModel M = mdl[m];
+    if (threadIdx.x == 0) {
+        double e_min = INFINITY;
+        for (int z = 0; z < Z; ++z) {
+            double d = __dsub_rn(feh_grid[z], M.feh_mean);
+            w[z] = __ddiv_rn(__dmul_rn(d, d), __dmul_rn(__dmul_rn(2.0, M.feh_sigma), M.feh_sigma));
+            if (w[z] < e_min) e_min = w[z];
+        }
+        double G = 0.0;
+        for (int z = 0; z < Z; ++z) { w[z] = expneg_basic(__dsub_rn(w[z], e_min)); G = __dadd_rn(G, w[z]); }
+        double G2 = 0.0;
+        for (int z = 0; z < Z; ++z) {
+            w[z] = __ddiv_rn(w[z], G);
+            if (w[z] < mdf_cut) w[z] = 0.0;
+            G2 = __dadd_rn(G2, w[z]);
+        }
+        for (int z = 0; z < Z; ++z) { w[z] = __ddiv_rn(w[z], G2); mdfw_out[(size_t)m * Z + z] = w[z]; }
+    }
+    __syncthreads();
+    const double zp[4] = {zp0, zp1, zp2, zp3};
+    for (int j = threadIdx.x; j < Jpad; j += blockDim.x) {
+        PointRec r;
+        r.T0 = 0xFFFFFFFFu; r.off = 0; r.len = 0; r.k0 = 0;
+        r.f[0] = r.f[1] = r.f[2] = r.f[3] = 0.f;
+        if (j < J) {
+            double lam = __dmul_rn(__dmul_rn(sfh[(size_t)m * A + age_idx[j]], w[feh_idx[j]]), imf_w[j]);
+            lambda_out[(size_t)m * J + j] = lam;
+            if (!(lam >= 0.0) || lam > PCMD_LAMBDA_MAX) atomicMin(status, PCMD_ERANGE);
+            for (int b = 0; b < B; ++b)  // fluxes according to the distance
+                r.f[b] = (float)pow(10.0, -0.4 * (absmag[(size_t)j * B + b] + M.dmod - zp[b]));
+        }
+        rec_out[(size_t)m * Jpad + j] = r;
+    }
+}
+
+// Range [k_lo, k_hi] of the relative pmf q[k] >= 2^-64 (R-C2 step 1), one thread per point.
+__global__ void k_table_range(const double *__restrict__ lambda, int J, int n_models,
+                              uint32_t *__restrict__ rawcnt, uint32_t *__restrict__ klo_out) {
+    int idx = blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= J * n_models) return;
+    int m = idx / J, j = idx - m * J;
+    double lam = lambda[idx];
+    uint32_t n = 0, klo = 0;
+    if (lam > 0.0 && lam <= PCMD_LAMBDA_MAX) {
+        long long mode = (long long)floor(lam), k_hi = mode, k_lo = mode;
+        double v = 1.0;
+        for (long long k = mode + 1;; ++k) {
+            v = __dmul_rn(v, __ddiv_rn(lam, (double)k));
+            if (v < TWO_M64) break;
+            k_hi = k;
+        }
+        v = 1.0;
+        for (long long k = mode - 1; k >= 0; --k) {
+            v = __dmul_rn(v, __ddiv_rn((double)(k + 1), lam));
+            if (v < TWO_M64) break;
+            k_lo = k;
+        }
+        n = (uint32_t)(k_hi - k_lo + 1);
+        klo = (uint32_t)k_lo;
+    }
+    rawcnt[(size_t)m * (J + 1) + j] = n;
+    klo_out[idx] = klo;
+}
+
+// In-place exclusive scan of cnt[m][0..J] (entry J receives the total), one block per model.
+__global__ void k_scan(uint32_t *__restrict__ cnt, int J, int64_t cap, int32_t *status) {
+    __shared__ uint32_t warp_sum[32];
+    __shared__ uint32_t carry;
+    uint32_t *c = cnt + (size_t)blockIdx.x * (J + 1);
+    if (threadIdx.x == 0) carry = 0;
+    __syncthreads();
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
+    for (int base = 0; base < J; base += blockDim.x) {
+        int j = base + threadIdx.x;
+        uint32_t v = (j < J) ? c[j] : 0, x = v;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) { uint32_t y = __shfl_up_sync(0xffffffffu, x, d); if (lane >= d) x += y; }
+        if (lane == 31) warp_sum[wid] = x;
+        __syncthreads();
+        if (wid == 0) {
+            uint32_t s = (lane < nw) ? warp_sum[lane] : 0;
+#pragma unroll
+            for (int d = 1; d < 32; d <<= 1) { uint32_t y = __shfl_up_sync(0xffffffffu, s, d); if (lane >= d) s += y; }
+            warp_sum[lane] = s;
+        }
+        __syncthreads();
+        uint32_t before = carry + (wid ? warp_sum[wid - 1] : 0) + (x - v);
+        if (j < J) c[j] = before;
+        __syncthreads();
+        if (threadIdx.x == blockDim.x - 1) carry = before + v;
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) {
+        c[J] = carry;
+        if ((int64_t)carry > cap) atomicMin(status, PCMD_ENOMEM);
+    }
+}
+
+// R-C2 steps 1-3 for one point per thread: q[k] by the two recurrences into scratch, S summed
+// in increasing k, thresholds T[k] = (uint64)((c/S) 2^32 + 0.5) written over q.  Also counts
+// the stored thresholds (0 < T < 2^32) and k0 = first k with T > 0.
+__global__ void k_table_fill(const double *__restrict__ lambda, int J, int n_models,
+                             const uint32_t *__restrict__ rawoff, const uint32_t *__restrict__ klo_in,
+                             double *__restrict__ qbuf, int64_t cap, uint32_t *__restrict__ stcnt,
+                             PointRec *__restrict__ rec, int Jpad) {
+    int idx = blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= J * n_models) return;
+    int m = idx / J, j = idx - m * J;
+    const uint32_t *ro = rawoff + (size_t)m * (J + 1);
+    uint32_t off = ro[j], n = ro[j + 1] - off, stored = 0, k0 = 0;
+    if (n > 0 && (int64_t)ro[J] <= cap) {
+        double lam = lambda[idx];
+        double *q = qbuf + (size_t)m * cap + off;
+        long long k_lo = klo_in[idx], mode = (long long)floor(lam), k_hi = k_lo + n - 1;
+        q[mode - k_lo] = 1.0;
+        double v = 1.0;
+        for (long long k = mode + 1; k <= k_hi; ++k) { v = __dmul_rn(v, __ddiv_rn(lam, (double)k)); q[k - k_lo] = v; }
+        v = 1.0;
+        for (long long k = mode - 1; k >= k_lo; --k) { v = __dmul_rn(v, __ddiv_rn((double)(k + 1), lam)); q[k - k_lo] = v; }
+        double S = 0.0;
+        for (uint32_t i = 0; i < n; ++i) S = __dadd_rn(S, q[i]);
+        double c = 0.0;
+        uint32_t zeros = 0;
+        for (uint32_t i = 0; i < n; ++i) {
+            c = __dadd_rn(c, q[i]);
+            unsigned long long t = __double2ull_rz(__dadd_rn(__dmul_rn(__ddiv_rn(c, S), TWO32), 0.5));
+            q[i] = __longlong_as_double((long long)t);  // q[i] is no longer needed
+            if (t == 0ull) zeros++;
+            else if (t < 4294967296ull) stored++;
+        }
+        k0 = (uint32_t)k_lo + zeros;
+    }
+    stcnt[(size_t)m * (J + 1) + j] = stored;
+    rec[(size_t)m * Jpad + j].k0 = k0;
+    rec[(size_t)m * Jpad + j].len = stored;
+}
+
+// Compacts the stored thresholds (minus 1) into the model's table and completes the records.
+__global__ void k_table_compact(int J, int n_models, const uint32_t *__restrict__ rawoff,
+                                const double *__restrict__ qbuf, int64_t cap,
+                                const uint32_t *__restrict__ stoff, uint32_t *__restrict__ tab,
+                                PointRec *__restrict__ rec, int Jpad) {
+    int idx = blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= J * n_models) return;
+    int m = idx / J, j = idx - m * J;
+    const uint32_t *ro = rawoff + (size_t)m * (J + 1);
+    const uint32_t *so = stoff + (size_t)m * (J + 1);
+    if ((int64_t)ro[J] > cap) return;
+    uint32_t off = ro[j], n = ro[j + 1] - off, dst = so[j];
+    const double *T = qbuf + (size_t)m * cap + off;
+    uint32_t *out = tab + (size_t)m * cap;
+    uint32_t w = dst;
+    for (uint32_t i = 0; i < n; ++i) {
+        unsigned long long t = (unsigned long long)__double_as_longlong(T[i]);
+        if (t != 0ull && t < 4294967296ull) out[w++] = (uint32_t)(t - 1ull);
+    }
+    PointRec *r = rec + (size_t)m * Jpad + j;
+    r->off = dst;
+    r->T0 = (w > dst) ? out[dst] : 0xFFFFFFFFu;
+}
+
+static int build_tables(pcmd_ctx *c, const double *d_lambda, int J, int n_models, uint32_t *rawcnt,
+                        uint32_t *klo, double *q, int64_t cap, uint32_t *stcnt, uint32_t *tab,
+                        PointRec *rec, int Jpad, cudaStream_t s) {
+    int total = J * n_models, tb = 128, gb = (total + tb - 1) / tb;
+    k_table_range<<<gb, tb, 0, s>>>(d_lambda, J, n_models, rawcnt, klo);
+    PCMD_LAUNCHED(c);
+    k_scan<<<n_models, 1024, 0, s>>>(rawcnt, J, cap, c->d_status);
+    PCMD_LAUNCHED(c);
+    k_table_fill<<<gb, tb, 0, s>>>(d_lambda, J, n_models, rawcnt, klo, q, cap, stcnt, rec, Jpad);
+    PCMD_LAUNCHED(c);
+    k_scan<<<n_models, 1024, 0, s>>>(stcnt, J, cap, c->d_status);
+    PCMD_LAUNCHED(c);
+    k_table_compact<<<gb, tb, 0, s>>>(J, n_models, rawcnt, q, cap, stcnt, tab, rec, Jpad);
+    PCMD_LAUNCHED(c);
+    return PCMD_OK;
+}
+
+int pcmd_launch_stage1(pcmd_ctx *c, int n_models, cudaStream_t s) {
+    k_weights<<<n_models, 256, c->Z * sizeof(double), s>>>(
+        c->d_model, c->d_sfh, c->d_feh_grid, c->d_age_idx, c->d_feh_idx, c->d_imf_w, c->d_absmag, c->A,
+        c->Z, c->J, c->Jpad, c->B, c->mdf_cut, c->zp[0], c->zp[1], c->zp[2], c->zp[3], c->d_mdfw,
+        c->d_lambda, c->d_rec, c->d_status);
+    PCMD_LAUNCHED(c);
+    return build_tables(c, c->d_lambda, c->J, n_models, c->d_rawcnt, c->d_klo, c->d_q, c->cap_raw,
+                        c->d_stcnt, c->d_tab, c->d_rec, c->Jpad, s);
+}
+
+// One sampler table per band for Poisson(sky_b) (R-Q11), built once at pcmd_create with the
+// same kernels (J = B "points", one "model").
+int pcmd_build_sky_tables(pcmd_ctx *c) {
+    const int B = c->B;
+    double maxsky = 0.0;
+    for (int b = 0; b < B; ++b) maxsky = c->sky[b] > maxsky ? c->sky[b] : maxsky;
+    int64_t cap = (int64_t)B * (int64_t)(20.0 * sqrt(maxsky) + 96.0);
+    double *d_lam = nullptr, *d_q = nullptr;
+    uint32_t *d_raw = nullptr, *d_klo = nullptr, *d_st = nullptr;
+    PointRec *d_rec = nullptr;
+    PCMD_CUDA(c, cudaMalloc(&d_lam, B * sizeof(double)));
+    PCMD_CUDA(c, cudaMalloc(&d_q, cap * sizeof(double)));
+    PCMD_CUDA(c, cudaMalloc(&d_raw, (B + 1) * sizeof(uint32_t)));
+    PCMD_CUDA(c, cudaMalloc(&d_st, (B + 1) * sizeof(uint32_t)));
+    PCMD_CUDA(c, cudaMalloc(&d_klo, B * sizeof(uint32_t)));
+    PCMD_CUDA(c, cudaMalloc(&d_rec, 4 * sizeof(PointRec)));
+    PCMD_CUDA(c, cudaMalloc(&c->d_sky_tab, cap * sizeof(uint32_t)));
+    PCMD_CUDA(c, cudaMemset(d_rec, 0, 4 * sizeof(PointRec)));
+    PCMD_CUDA(c, cudaMemcpy(d_lam, c->sky, B * sizeof(double), cudaMemcpyHostToDevice));
+    int rc = build_tables(c, d_lam, B, 1, d_raw, d_klo, d_q, cap, d_st, c->d_sky_tab, d_rec, 4, 0);
+    if (rc) return rc;
+    PointRec h[4];
+    PCMD_CUDA(c, cudaMemcpy(h, d_rec, 4 * sizeof(PointRec), cudaMemcpyDeviceToHost));
+    c->sky_cap = (uint32_t)cap;
+    for (int b = 0; b < B; ++b) c->sky_rec[b] = h[b];   // (off, len, k0) of each band's table
+    cudaFree(d_lam); cudaFree(d_q); cudaFree(d_raw); cudaFree(d_st); cudaFree(d_klo); cudaFree(d_rec);
+    return PCMD_OK;
+}
