@@ -155,6 +155,13 @@ int  pcmd_debug_philox(uint64_t seed, const uint32_t *h_ctr, int64_t n, uint32_t
  * PCMD_ERANGE / PCMD_ENOMEM raised by a kernel (lambda too large, sampler-table scratch full). */
 int  pcmd_status(pcmd_ctx *ctx, void *cuda_stream);
 int  pcmd_last_cuda_error(const pcmd_ctx *ctx);
+/* Per-stage device timing.  pcmd_profile(ctx, 1) makes the following pcmd_simulate / pcmd_hess /
+ * pcmd_loglike calls record CUDA events on the caller's stream around each stage;
+ * pcmd_stage_ms waits for the events of the LAST such calls and writes h_ms[5] HOST float32
+ * milliseconds: stage 1 (weights + sampler tables), stage 2 (+ dust epilogue), stages 4-5
+ * (convolution + noise + magnitudes), stage 6, stage 7; -1 for a stage not run since enabling. */
+int  pcmd_profile(pcmd_ctx *ctx, int32_t enable);
+int  pcmd_stage_ms(pcmd_ctx *ctx, float *h_ms);
 /* Kernels launched on behalf of this ctx since pcmd_create (bench.py's gpu_launches). */
 int64_t pcmd_launch_count(const pcmd_ctx *ctx);
 /* Stage-2 variant: 0 = default choice; see DESIGN.md "Stage 2".  Returns the previous value. */

@@ -89,6 +89,8 @@ def lib():
         L.pcmd_launch_count.argtypes = [vp]
         L.pcmd_launch_count.restype = i64
         L.pcmd_set_option.argtypes = [vp, C.c_char_p, i64]
+        L.pcmd_profile.argtypes = [vp, i32]
+        L.pcmd_stage_ms.argtypes = [vp, vp]
         _lib = L
     return _lib
 
@@ -265,6 +267,19 @@ class Pcmd:
 
     def status(self):
         return int(lib().pcmd_status(self._ctx, self._stream()))
+
+    def profile(self, enable=True):
+        rc = lib().pcmd_profile(self._ctx, int(bool(enable)))
+        if rc:
+            raise PcmdError(rc, "pcmd_profile")
+
+    def stage_ms(self):
+        """Milliseconds of stages (1, 2, 4-5, 6, 7) of the last profiled calls (synchronises)."""
+        ms = np.zeros(5, dtype=np.float32)
+        rc = lib().pcmd_stage_ms(self._ctx, _np(ms))
+        if rc:
+            raise PcmdError(rc, "pcmd_stage_ms")
+        return ms
 
     def launch_count(self):
         return int(lib().pcmd_launch_count(self._ctx))

@@ -184,6 +184,7 @@ extern "C" void pcmd_destroy(pcmd_ctx *c) {
     cudaFree(c->d_hess_data); cudaFree(c->d_data_stats);
     if (c->h_pin) cudaFreeHost(c->h_pin);
     if (c->stage_ev_valid) cudaEventDestroy(c->stage_ev);
+    if (c->prof_made) for (int i = 0; i < 8; ++i) cudaEventDestroy(c->prof_ev[i]);
     free(c->h_imf_w);
     delete c;
 }
@@ -248,18 +249,28 @@ extern "C" int pcmd_simulate(pcmd_ctx *c, const pcmd_params *params, int32_t n_m
     PCMD_CUDA(c, cudaEventRecord(c->stage_ev, s));
     PCMD_CUDA(c, cudaMemsetAsync(c->d_status, 0, sizeof(int32_t), s));
     c->last_models = n_models;
+    PCMD_PROF(c, 0, s);
     if ((rc = pcmd_launch_stage1(c, n_models, s))) return rc;
+    PCMD_PROF(c, 1, s);
     if ((rc = pcmd_launch_stage2(c, n_models, seed, model_index0, d_flux_raw, d_count_hash, d_count_total, s))) return rc;
+    PCMD_PROF(c, 2, s);
     if (c->tap_dust)
         PCMD_CUDA(c, cudaMemcpyAsync(c->tap_dust, c->d_fdust, (size_t)n_models * c->B * c->P * sizeof(float),
                                      cudaMemcpyDeviceToDevice, s));
-    return pcmd_launch_conv_noise(c, n_models, seed, model_index0, d_mag, s);
+    if ((rc = pcmd_launch_conv_noise(c, n_models, seed, model_index0, d_mag, s))) return rc;
+    PCMD_PROF(c, 3, s);
+    return PCMD_OK;
 }
 
 extern "C" int pcmd_hess(pcmd_ctx *c, const float *d_mag, int32_t n_models, uint32_t *d_hess,
                          pcmd_hess_stats *d_stats, void *cuda_stream) {
     if (!c || !d_mag || !d_hess || n_models < 1 || c->n_hess < 1) return PCMD_EINVAL;
-    return pcmd_launch_hess(c, d_mag, n_models, d_hess, d_stats, (cudaStream_t)cuda_stream);
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    PCMD_PROF(c, 4, s);
+    int rc = pcmd_launch_hess(c, d_mag, n_models, d_hess, d_stats, s);
+    if (rc) return rc;
+    PCMD_PROF(c, 5, s);
+    return PCMD_OK;
 }
 
 extern "C" int pcmd_loglike(pcmd_ctx *c, const uint32_t *d_hess_model, const pcmd_hess_stats *d_stats,
@@ -269,8 +280,13 @@ extern "C" int pcmd_loglike(pcmd_ctx *c, const uint32_t *d_hess_model, const pcm
     if (!c || !d_hess_model || !d_hess_data || !d_loglike || n_models < 1 || c->n_hess < 1) return PCMD_EINVAL;
     if (like_mode < PCMD_LIKE_POISSON || like_mode > PCMD_LIKE_GAUSS_LITERAL) return PCMD_EINVAL;
     if (like_mode != PCMD_LIKE_POISSON && (!d_stats || !d_data_stats)) return PCMD_EINVAL;
-    return pcmd_launch_loglike(c, d_hess_model, d_stats, n_models, d_hess_data, d_data_stats, like_mode,
-                               d_loglike, (cudaStream_t)cuda_stream);
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    PCMD_PROF(c, 6, s);
+    int rc = pcmd_launch_loglike(c, d_hess_model, d_stats, n_models, d_hess_data, d_data_stats, like_mode,
+                                 d_loglike, s);
+    if (rc) return rc;
+    PCMD_PROF(c, 7, s);
+    return PCMD_OK;
 }
 
 extern "C" int64_t pcmd_hess_bins_total(const pcmd_ctx *c) { return c ? c->hess_bins : 0; }
@@ -316,9 +332,9 @@ extern "C" int pcmd_evaluate_host(pcmd_ctx *c, const pcmd_params *params, int32_
     }
     int rc = pcmd_simulate(c, params, n_models, seed, model_index0, c->d_mag, nullptr, nullptr, nullptr, cuda_stream);
     if (rc) return rc;
-    if ((rc = pcmd_launch_hess(c, c->d_mag, n_models, c->d_hessbuf, c->d_statbuf, s))) return rc;
-    if ((rc = pcmd_launch_loglike(c, c->d_hessbuf, c->d_statbuf, n_models, c->d_hess_data,
-                                  h_data_stats ? c->d_data_stats : nullptr, like_mode, c->d_lnl, s)))
+    if ((rc = pcmd_hess(c, c->d_mag, n_models, c->d_hessbuf, c->d_statbuf, cuda_stream))) return rc;
+    if ((rc = pcmd_loglike(c, c->d_hessbuf, c->d_statbuf, n_models, c->d_hess_data,
+                           h_data_stats ? c->d_data_stats : nullptr, like_mode, c->d_lnl, cuda_stream)))
         return rc;
     PCMD_CUDA(c, cudaMemcpyAsync(p_l, c->d_lnl, (size_t)n_models * sizeof(double), cudaMemcpyDeviceToHost, s));
     if (h_hess_out)
@@ -402,6 +418,30 @@ extern "C" int pcmd_status(pcmd_ctx *c, void *cuda_stream) {
     int32_t st = 0;
     PCMD_CUDA(c, cudaMemcpy(&st, c->d_status, sizeof(int32_t), cudaMemcpyDeviceToHost));
     return st;
+}
+
+extern "C" int pcmd_profile(pcmd_ctx *c, int32_t enable) {
+    if (!c) return PCMD_EINVAL;
+    if (enable && !c->prof_made) {
+        for (int i = 0; i < 8; ++i) PCMD_CUDA(c, cudaEventCreate(&c->prof_ev[i]));
+        c->prof_made = 1;
+    }
+    c->prof_on = enable != 0;
+    c->prof_seen = 0;
+    return PCMD_OK;
+}
+
+extern "C" int pcmd_stage_ms(pcmd_ctx *c, float *h_ms) {
+    if (!c || !h_ms || !c->prof_made) return PCMD_EINVAL;
+    static const int span[5][2] = {{0, 1}, {1, 2}, {2, 3}, {4, 5}, {6, 7}};
+    for (int i = 0; i < 5; ++i) {
+        h_ms[i] = -1.f;
+        const uint32_t need = (1u << span[i][0]) | (1u << span[i][1]);
+        if ((c->prof_seen & need) != need) continue;
+        PCMD_CUDA(c, cudaEventSynchronize(c->prof_ev[span[i][1]]));
+        PCMD_CUDA(c, cudaEventElapsedTime(&h_ms[i], c->prof_ev[span[i][0]], c->prof_ev[span[i][1]]));
+    }
+    return PCMD_OK;
 }
 
 extern "C" int pcmd_last_cuda_error(const pcmd_ctx *c) { return c ? c->last_cuda : 0; }

@@ -73,7 +73,17 @@ struct pcmd_ctx {
     int64_t launches;
     int sm_count;
     cudaEvent_t stage_ev; int stage_ev_valid;
+    // per-stage timing (pcmd_profile): events recorded on the caller's stream around each stage
+    cudaEvent_t prof_ev[8]; int prof_on, prof_made; uint32_t prof_seen;
 };
+
+#define PCMD_PROF(ctx, i, s)                                              \
+    do {                                                                  \
+        if ((ctx)->prof_on) {                                             \
+            PCMD_CUDA(ctx, cudaEventRecord((ctx)->prof_ev[i], s));        \
+            (ctx)->prof_seen |= 1u << (i);                                \
+        }                                                                 \
+    } while (0)
 
 // error helpers ---------------------------------------------------------------------------
 #define PCMD_CUDA(ctx, call)                                              \
