@@ -35,7 +35,8 @@ extern "C" const char *pcmd_strerror(int code) {
 static void free_scratch(pcmd_ctx *c) {
     cudaFree(c->d_sfh); cudaFree(c->d_model); cudaFree(c->d_mdfw); cudaFree(c->d_lambda);
     cudaFree(c->d_rawcnt); cudaFree(c->d_klo); cudaFree(c->d_q); cudaFree(c->d_stcnt);
-    cudaFree(c->d_tab); cudaFree(c->d_rec); cudaFree(c->d_fdust);
+    cudaFree(c->d_tab); cudaFree(c->d_rec); cudaFree(c->d_fdust); cudaFree(c->d_grp); cudaFree(c->d_seg);
+    c->d_grp = nullptr; c->d_seg = nullptr;
     if (c->h_stage) cudaFreeHost(c->h_stage);
     c->d_sfh = nullptr; c->d_model = nullptr; c->d_mdfw = nullptr; c->d_lambda = nullptr;
     c->d_rawcnt = nullptr; c->d_klo = nullptr; c->d_q = nullptr; c->d_stcnt = nullptr;
@@ -62,6 +63,8 @@ static int ensure_scratch(pcmd_ctx *c, int n_models, int64_t cap_raw) {
     PCMD_CUDA(c, cudaMalloc(&c->d_tab, (size_t)nm * cr * sizeof(uint32_t)));
     PCMD_CUDA(c, cudaMalloc(&c->d_rec, (size_t)nm * Jp * sizeof(PointRec)));
     PCMD_CUDA(c, cudaMalloc(&c->d_fdust, (size_t)nm * c->B * c->P * sizeof(float)));
+    PCMD_CUDA(c, cudaMalloc(&c->d_grp, (size_t)nm * (Jp / 4) * sizeof(GroupRec)));
+    PCMD_CUDA(c, cudaMalloc(&c->d_seg, (size_t)nm * sizeof(SegTable)));
     c->h_stage_bytes = (size_t)nm * (c->A * sizeof(double) + sizeof(DevModel));
     PCMD_CUDA(c, cudaMallocHost(&c->h_stage, c->h_stage_bytes));
     c->cap_models = nm; c->cap_raw = cr;
@@ -162,11 +165,12 @@ extern "C" int pcmd_create(pcmd_ctx **out, const pcmd_config *cfg) {
         TRY(upload(c, &c->d_hess_spec, dh, (size_t)cfg->n_hess));
     }
     {
-        cudaError_t e = cudaMalloc(&c->d_status, sizeof(int32_t));
-        if (e == cudaSuccess) e = cudaMemset(c->d_status, 0, sizeof(int32_t));
+        cudaError_t e = cudaMalloc(&c->d_status, 2 * sizeof(int32_t));   // [status, stage-2 unit counter]
+        if (e == cudaSuccess) e = cudaMemset(c->d_status, 0, 2 * sizeof(int32_t));
         if (e != cudaSuccess) { c->last_cuda = (int)e; pcmd_destroy(c); return PCMD_ECUDA; }
     }
     TRY(pcmd_build_sky_tables(c));
+    TRY(pcmd_stage2_occupancy(c));
 #undef TRY
     cudaDeviceSynchronize();
     *out = c;
@@ -179,7 +183,7 @@ extern "C" void pcmd_destroy(pcmd_ctx *c) {
     free_scratch(c);
     cudaFree(c->d_age_idx); cudaFree(c->d_feh_idx); cudaFree(c->d_imf_w); cudaFree(c->d_absmag);
     cudaFree(c->d_feh_grid); cudaFree(c->d_psf); cudaFree(c->d_mult); cudaFree(c->d_hess_spec);
-    cudaFree(c->d_sky_tab); cudaFree(c->d_status); cudaFree(c->d_part);
+    cudaFree(c->d_sky_tab); cudaFree(c->d_status); cudaFree(c->d_hpart); cudaFree(c->d_part);
     cudaFree(c->d_mag); cudaFree(c->d_hessbuf); cudaFree(c->d_statbuf); cudaFree(c->d_lnl);
     cudaFree(c->d_hess_data); cudaFree(c->d_data_stats);
     if (c->h_pin) cudaFreeHost(c->h_pin);
@@ -220,6 +224,15 @@ static int stage_params(pcmd_ctx *c, const pcmd_params *params, int n_models, cu
     if (cap > 0xFFFFFFF0ll) return PCMD_ERANGE;
     int rc = ensure_scratch(c, n_models, cap);
     if (rc) return rc;
+    c->seg_budget = pcmd_stage2_seg_budget(c, n_models);
+    c->seg_cap = c->seg_budget + S2_NCLASS;
+    const int64_t need = (int64_t)n_models * c->seg_cap * c->B * c->P;
+    if (need > c->part_elems) {
+        cudaDeviceSynchronize();
+        cudaFree(c->d_part); c->d_part = nullptr; c->part_elems = 0;
+        PCMD_CUDA(c, cudaMalloc(&c->d_part, (size_t)need * sizeof(float)));
+        c->part_elems = need;
+    }
     double *hs = c->h_stage;
     DevModel *hm = reinterpret_cast<DevModel *>(hs + (size_t)n_models * c->A);
     for (int i = 0; i < n_models; ++i) {
@@ -247,7 +260,7 @@ extern "C" int pcmd_simulate(pcmd_ctx *c, const pcmd_params *params, int32_t n_m
         c->stage_ev_valid = 1;
     }
     PCMD_CUDA(c, cudaEventRecord(c->stage_ev, s));
-    PCMD_CUDA(c, cudaMemsetAsync(c->d_status, 0, sizeof(int32_t), s));
+    PCMD_CUDA(c, cudaMemsetAsync(c->d_status, 0, 2 * sizeof(int32_t), s));
     c->last_models = n_models;
     PCMD_PROF(c, 0, s);
     if ((rc = pcmd_launch_stage1(c, n_models, s))) return rc;

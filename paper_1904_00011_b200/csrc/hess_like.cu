@@ -90,11 +90,11 @@ int pcmd_launch_hess(pcmd_ctx *c, const float *d_mag, int n_models, uint32_t *d_
                      pcmd_hess_stats *d_stats, cudaStream_t s) {
     const int nblk = (int)((c->P + HS_PIX_PER_BLOCK - 1) / HS_PIX_PER_BLOCK);
     const int64_t need = (int64_t)n_models * c->n_hess * nblk;
-    if (need > c->part_cap) {
-        if (c->d_part) cudaFree(c->d_part);
-        c->d_part = nullptr; c->part_cap = 0;
-        PCMD_CUDA(c, cudaMalloc(&c->d_part, need * sizeof(pcmd_hess_stats)));
-        c->part_cap = need;
+    if (need > c->hpart_cap) {
+        if (c->d_hpart) cudaFree(c->d_hpart);
+        c->d_hpart = nullptr; c->hpart_cap = 0;
+        PCMD_CUDA(c, cudaMalloc(&c->d_hpart, need * sizeof(pcmd_hess_stats)));
+        c->hpart_cap = need;
     }
     PCMD_CUDA(c, cudaMemsetAsync(d_hess, 0, (size_t)n_models * c->hess_bins * sizeof(uint32_t), s));
     int maxbins = 0;
@@ -108,14 +108,14 @@ int pcmd_launch_hess(pcmd_ctx *c, const float *d_mag, int n_models, uint32_t *d_
             smem_set = smem;
         }
         k_hess<true><<<grid, HS_THREADS, smem, s>>>(d_mag, c->B, c->P, c->d_hess_spec, c->n_hess,
-                                                    c->hess_bins, d_hess, c->d_part);
+                                                    c->hess_bins, d_hess, c->d_hpart);
     } else {
         k_hess<false><<<grid, HS_THREADS, 0, s>>>(d_mag, c->B, c->P, c->d_hess_spec, c->n_hess,
-                                                  c->hess_bins, d_hess, c->d_part);
+                                                  c->hess_bins, d_hess, c->d_hpart);
     }
     PCMD_LAUNCHED(c);
     if (d_stats) {
-        k_hess_stats<<<n_models * c->n_hess, 32, 0, s>>>(c->d_part, nblk, d_stats);
+        k_hess_stats<<<n_models * c->n_hess, 32, 0, s>>>(c->d_hpart, nblk, d_stats);
         PCMD_LAUNCHED(c);
     }
     return PCMD_OK;

@@ -15,6 +15,21 @@ struct __align__(16) PointRec {
     float f[4];     // flux of one star in each band (electrons), unused bands 0
 };
 
+// Stage-2 work layout.  Groups of four consecutive isochrone points (one
+// Philox call, R-C1) are classified by how many sampler thresholds decide almost every draw and
+// sorted by class; a class is cut into segments; one (model, pixel tile, segment) is a work unit.
+#define S2_NCLASS 4        // 0 generic (table search), 1: four inline thresholds, 2: two, 3: one
+#define S2_SEG_MAX 40      // segments per model (all classes together)
+struct __align__(16) GroupRec {      // 160 bytes
+    uint32_t g_orig, cls, pad0, pad1; // original group index (Philox counter word 1), class
+    uint32_t T[5][4];                 // T[i][w]: (i+1)-th stored threshold minus 1 of point w; 0xFFFFFFFF if none
+    float f[4][4];                    // f[w][b]: flux of one star of point w in band b
+};
+struct SegTable {                     // per model
+    int32_t n_seg, pad;
+    int32_t g_lo[S2_SEG_MAX], g_hi[S2_SEG_MAX], cls[S2_SEG_MAX];  // sorted-group ranges
+};
+
 struct DevHess {
     int32_t band_plus, band_minus, band_y, nx, ny;
     float x_lo, y_lo, inv_dx, inv_dy;
@@ -57,9 +72,13 @@ struct pcmd_ctx {
     uint32_t *d_tab;       // [cap_models][cap_raw] stored thresholds minus 1
     PointRec *d_rec;       // [cap_models][Jpad]
     float *d_fdust;        // [cap_models][B][P]
+    GroupRec *d_grp;       // [cap_models][Jpad/4] class-sorted group records
+    SegTable *d_seg;       // [cap_models]
+    float *d_part;  int64_t part_elems;  // stage-2 partial fluxes [cap_models][seg_cap][B][P]
+    int32_t seg_budget, seg_cap, s2_ctas_per_sm;
     int32_t *d_status;     // device status word
     // hess / loglike scratch
-    pcmd_hess_stats *d_part; int64_t part_cap;   // per-block partial stats
+    pcmd_hess_stats *d_hpart; int64_t hpart_cap; // per-block partial stats
     // evaluate_host scratch
     float *d_mag; uint32_t *d_hessbuf; pcmd_hess_stats *d_statbuf; double *d_lnl;
     uint32_t *d_hess_data; pcmd_hess_stats *d_data_stats;
@@ -141,6 +160,8 @@ int pcmd_launch_stage1(pcmd_ctx *c, int n_models, cudaStream_t s);
 int pcmd_build_sky_tables(pcmd_ctx *c);
 int pcmd_launch_stage2(pcmd_ctx *c, int n_models, uint64_t seed, uint32_t model0, float *d_flux_raw,
                        uint64_t *d_hash, uint32_t *d_total, cudaStream_t s);
+int pcmd_stage2_seg_budget(const pcmd_ctx *c, int n_models);
+int pcmd_stage2_occupancy(pcmd_ctx *c);
 int pcmd_launch_conv_noise(pcmd_ctx *c, int n_models, uint64_t seed, uint32_t model0, float *d_mag,
                            cudaStream_t s);
 int pcmd_launch_hess(pcmd_ctx *c, const float *d_mag, int n_models, uint32_t *d_hess,

@@ -193,6 +193,103 @@ __global__ void k_table_compact(int J, int n_models, const uint32_t *__restrict_
     r->T0 = (w > dst) ? out[dst] : 0xFFFFFFFFu;
 }
 
+
+// ---------------------------------------------------------------------------------------------
+// Stage-2 work layout: classify the groups of four points, sort them by class, cut segments.
+// One block per model.  Class of a point: the smallest L in {1,2,4} such that k0 = 0 and the
+// probability of more than L stars is below 2^-10 (its (L+1)-th threshold is above
+// 2^32 (1 - 2^-10)), else generic.  The class of a group is the most expensive of its points.
+#define S2_OVF_THR 4290772991u   /* 2^32 (1 - 2^-10) - 1 */
+
+__device__ __forceinline__ int point_class(const PointRec &r, const uint32_t *__restrict__ tab) {
+    if (r.len == 0 && r.k0 == 0) return 4;               // never a star
+    if (r.k0 != 0) return 0;
+    if (r.len <= 1 || tab[r.off + 1] >= S2_OVF_THR) return 3;
+    if (r.len <= 2 || tab[r.off + 2] >= S2_OVF_THR) return 2;
+    if (r.len <= 4 || tab[r.off + 4] >= S2_OVF_THR) return 1;
+    return 0;
+}
+
+__global__ void __launch_bounds__(1024) k_group_sort(const PointRec *__restrict__ rec_all,
+                                                     const uint32_t *__restrict__ tab_all, int64_t cap,
+                                                     int Jpad, int seg_budget, GroupRec *__restrict__ grp_all,
+                                                     SegTable *__restrict__ seg_all) {
+    __shared__ uint32_t warp_sum[32];
+    __shared__ uint32_t carry, cls_start[S2_NCLASS + 1];
+    const int m = blockIdx.x, n_groups = Jpad >> 2;
+    const PointRec *rec = rec_all + (size_t)m * Jpad;
+    const uint32_t *tab = tab_all + (size_t)m * cap;
+    GroupRec *grp = grp_all + (size_t)m * n_groups;
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
+    if (threadIdx.x == 0) { carry = 0; cls_start[0] = 0; }
+    __syncthreads();
+    for (int c = 0; c < S2_NCLASS; ++c) {
+        for (int base = 0; base < n_groups; base += blockDim.x) {
+            const int g = base + threadIdx.x;
+            int cls = 5;
+            if (g < n_groups) {
+                cls = 4;
+#pragma unroll
+                for (int w = 0; w < 4; ++w) cls = min(cls, point_class(rec[4 * g + w], tab));
+            }
+            const uint32_t v = (cls == c) ? 1u : 0u;
+            uint32_t x = v;
+#pragma unroll
+            for (int d = 1; d < 32; d <<= 1) { uint32_t y = __shfl_up_sync(0xffffffffu, x, d); if (lane >= d) x += y; }
+            if (lane == 31) warp_sum[wid] = x;
+            __syncthreads();
+            if (wid == 0) {
+                uint32_t sv = (lane < nw) ? warp_sum[lane] : 0;
+#pragma unroll
+                for (int d = 1; d < 32; d <<= 1) { uint32_t y = __shfl_up_sync(0xffffffffu, sv, d); if (lane >= d) sv += y; }
+                warp_sum[lane] = sv;
+            }
+            __syncthreads();
+            const uint32_t pos = carry + (wid ? warp_sum[wid - 1] : 0) + (x - v);
+            if (v) {
+                GroupRec o;
+                o.g_orig = (uint32_t)g; o.cls = (uint32_t)c; o.pad0 = o.pad1 = 0;
+#pragma unroll
+                for (int w = 0; w < 4; ++w) {
+                    const PointRec r = rec[4 * g + w];
+#pragma unroll
+                    for (int i = 0; i < 5; ++i) o.T[i][w] = ((uint32_t)i < r.len) ? tab[r.off + i] : 0xFFFFFFFFu;
+#pragma unroll
+                    for (int b = 0; b < 4; ++b) o.f[w][b] = r.f[b];
+                }
+                grp[pos] = o;
+            }
+            __syncthreads();
+            if (threadIdx.x == blockDim.x - 1) carry = pos + v;
+            __syncthreads();
+        }
+        if (threadIdx.x == 0) cls_start[c + 1] = carry;
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) {
+        // segments: each class gets a share of seg_budget proportional to its estimated cost
+        const float wgt[S2_NCLASS] = {3.0f, 1.5f, 1.15f, 1.0f};
+        float total = 0.f;
+        for (int c = 0; c < S2_NCLASS; ++c) total += wgt[c] * (float)(cls_start[c + 1] - cls_start[c]);
+        SegTable t;
+        t.n_seg = 0; t.pad = 0;
+        for (int c = 0; c < S2_NCLASS; ++c) {
+            const int n = (int)(cls_start[c + 1] - cls_start[c]);
+            if (n == 0) continue;
+            int k = (int)(wgt[c] * (float)n / total * (float)seg_budget + 0.5f);
+            k = max(1, min(k, min(n, S2_SEG_MAX - S2_NCLASS)));
+            for (int i = 0; i < k && t.n_seg < S2_SEG_MAX; ++i) {
+                t.g_lo[t.n_seg] = (int)cls_start[c] + (int)((int64_t)n * i / k);
+                t.g_hi[t.n_seg] = (int)cls_start[c] + (int)((int64_t)n * (i + 1) / k);
+                t.cls[t.n_seg] = c;
+                t.n_seg++;
+            }
+        }
+        for (int i = t.n_seg; i < S2_SEG_MAX; ++i) { t.g_lo[i] = t.g_hi[i] = 0; t.cls[i] = 0; }
+        seg_all[m] = t;
+    }
+}
+
 static int build_tables(pcmd_ctx *c, const double *d_lambda, int J, int n_models, uint32_t *rawcnt,
                         uint32_t *klo, double *q, int64_t cap, uint32_t *stcnt, uint32_t *tab,
                         PointRec *rec, int Jpad, cudaStream_t s) {
@@ -216,8 +313,13 @@ int pcmd_launch_stage1(pcmd_ctx *c, int n_models, cudaStream_t s) {
         c->Z, c->J, c->Jpad, c->B, c->mdf_cut, c->zp[0], c->zp[1], c->zp[2], c->zp[3], c->d_mdfw,
         c->d_lambda, c->d_rec, c->d_status);
     PCMD_LAUNCHED(c);
-    return build_tables(c, c->d_lambda, c->J, n_models, c->d_rawcnt, c->d_klo, c->d_q, c->cap_raw,
-                        c->d_stcnt, c->d_tab, c->d_rec, c->Jpad, s);
+    int rc = build_tables(c, c->d_lambda, c->J, n_models, c->d_rawcnt, c->d_klo, c->d_q, c->cap_raw,
+                          c->d_stcnt, c->d_tab, c->d_rec, c->Jpad, s);
+    if (rc) return rc;
+    k_group_sort<<<n_models, 1024, 0, s>>>(c->d_rec, c->d_tab, c->cap_raw, c->Jpad, c->seg_budget, c->d_grp,
+                                           c->d_seg);
+    PCMD_LAUNCHED(c);
+    return PCMD_OK;
 }
 
 // One sampler table per band for Poisson(sky_b) (R-Q11), built once at pcmd_create with the
