@@ -18,8 +18,15 @@ struct __align__(16) PointRec {
 // Stage-2 work layout.  Groups of four consecutive isochrone points (one
 // Philox call, R-C1) are classified by how many sampler thresholds decide almost every draw and
 // sorted by class; a class is cut into segments; one (model, pixel tile, segment) is a work unit.
-#define S2_NCLASS 4        // 0 generic (table search), 1: four inline thresholds, 2: two, 3: one
-#define S2_SEG_MAX 40      // segments per model (all classes together)
+#define S2_NCLASS 7        // classes, most expensive first:
+#define S2_CLS_D9 1        //   0 bisection in global memory (tables longer than 511)
+#define S2_CLS_D7 2        //   1-3 branch-free search of a padded table of 2^D words in shared memory
+#define S2_CLS_D5 3
+#define S2_CLS_L4 4        //   4-6 L inline thresholds decide the draw (more stars: probability < 2^-10)
+#define S2_CLS_L2 5
+#define S2_CLS_L1 6
+#define S2_CLS_NONE 7      //   no point of the group can have a star: dropped
+#define S2_SEG_MAX 48      // segments per model (all classes together)
 struct __align__(16) GroupRec {      // 160 bytes
     uint32_t g_orig, cls, pad0, pad1; // original group index (Philox counter word 1), class
     uint32_t T[5][4];                 // T[i][w]: (i+1)-th stored threshold minus 1 of point w; 0xFFFFFFFF if none
@@ -28,6 +35,8 @@ struct __align__(16) GroupRec {      // 160 bytes
 struct SegTable {                     // per model
     int32_t n_seg, pad;
     int32_t g_lo[S2_SEG_MAX], g_hi[S2_SEG_MAX], cls[S2_SEG_MAX];  // sorted-group ranges
+    int32_t cls_start[S2_NCLASS + 1], first_d;                    // class ranges; first D class kept in the arena
+    int64_t arena_off[S2_NCLASS];                                 // word offset of a class's padded tables
 };
 
 struct DevHess {
@@ -74,6 +83,8 @@ struct pcmd_ctx {
     float *d_fdust;        // [cap_models][B][P]
     GroupRec *d_grp;       // [cap_models][Jpad/4] class-sorted group records
     SegTable *d_seg;       // [cap_models]
+    uint8_t *d_gcls;       // [cap_models][Jpad/4] class of each group (original order)
+    uint32_t *d_arena; int64_t arena_cap;  // [cap_models][arena_cap] padded search tables of the D classes
     float *d_part;  int64_t part_elems;  // stage-2 partial fluxes [cap_models][seg_cap][B][P]
     int32_t seg_budget, seg_cap, s2_ctas_per_sm;
     int32_t *d_status;     // device status word

@@ -195,98 +195,166 @@ __global__ void k_table_compact(int J, int n_models, const uint32_t *__restrict_
 
 
 // ---------------------------------------------------------------------------------------------
-// Stage-2 work layout: classify the groups of four points, sort them by class, cut segments.
-// One block per model.  Class of a point: the smallest L in {1,2,4} such that k0 = 0 and the
-// probability of more than L stars is below 2^-10 (its (L+1)-th threshold is above
-// 2^32 (1 - 2^-10)), else generic.  The class of a group is the most expensive of its points.
+// Stage-2 work layout: classify the groups of four points, sort them by class, cut segments, and
+// lay out the padded search tables of the D classes.  One block per model.
+// Class of a point:  L1/L2/L4: k0 = 0 and the probability of more than L stars is below 2^-10
+// (its (L+1)-th threshold is above 2^32 (1 - 2^-10)): L inline compares decide the draw;
+// D5/D7/D9: table of at most 2^D - 1 thresholds, searched branch-free in shared memory;
+// class 0: longer tables, bisection in global memory.  A group takes the most expensive class
+// of its four points.
 #define S2_OVF_THR 4290772991u   /* 2^32 (1 - 2^-10) - 1 */
 
 __device__ __forceinline__ int point_class(const PointRec &r, const uint32_t *__restrict__ tab) {
-    if (r.len == 0 && r.k0 == 0) return 4;               // never a star
-    if (r.k0 != 0) return 0;
-    if (r.len <= 1 || tab[r.off + 1] >= S2_OVF_THR) return 3;
-    if (r.len <= 2 || tab[r.off + 2] >= S2_OVF_THR) return 2;
-    if (r.len <= 4 || tab[r.off + 4] >= S2_OVF_THR) return 1;
+    if (r.len == 0 && r.k0 == 0) return S2_CLS_NONE;      // never a star
+    if (r.k0 == 0) {
+        if (r.len <= 1 || tab[r.off + 1] >= S2_OVF_THR) return S2_CLS_L1;
+        if (r.len <= 2 || tab[r.off + 2] >= S2_OVF_THR) return S2_CLS_L2;
+        if (r.len <= 4 || tab[r.off + 4] >= S2_OVF_THR) return S2_CLS_L4;
+    }
+    if (r.len <= 31) return S2_CLS_D5;
+    if (r.len <= 127) return S2_CLS_D7;
+    if (r.len <= 511) return S2_CLS_D9;
     return 0;
 }
 
 __global__ void __launch_bounds__(1024) k_group_sort(const PointRec *__restrict__ rec_all,
                                                      const uint32_t *__restrict__ tab_all, int64_t cap,
-                                                     int Jpad, int seg_budget, GroupRec *__restrict__ grp_all,
+                                                     int Jpad, int seg_budget, int64_t arena_cap,
+                                                     uint8_t *__restrict__ cls_all, GroupRec *__restrict__ grp_all,
                                                      SegTable *__restrict__ seg_all) {
-    __shared__ uint32_t warp_sum[32];
-    __shared__ uint32_t carry, cls_start[S2_NCLASS + 1];
+    __shared__ uint32_t wcnt[32][S2_NCLASS];
+    __shared__ uint32_t count[S2_NCLASS + 1], carry[S2_NCLASS], cls_start[S2_NCLASS + 1];
     const int m = blockIdx.x, n_groups = Jpad >> 2;
     const PointRec *rec = rec_all + (size_t)m * Jpad;
     const uint32_t *tab = tab_all + (size_t)m * cap;
     GroupRec *grp = grp_all + (size_t)m * n_groups;
+    uint8_t *gcls = cls_all + (size_t)m * n_groups;
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
-    if (threadIdx.x == 0) { carry = 0; cls_start[0] = 0; }
+    if (threadIdx.x <= S2_NCLASS) count[threadIdx.x] = 0;
     __syncthreads();
-    for (int c = 0; c < S2_NCLASS; ++c) {
-        for (int base = 0; base < n_groups; base += blockDim.x) {
-            const int g = base + threadIdx.x;
-            int cls = 5;
-            if (g < n_groups) {
-                cls = 4;
+    // pass 1: class of every group, class populations
+    for (int g = threadIdx.x; g < n_groups; g += blockDim.x) {
+        int cls = S2_CLS_NONE;
 #pragma unroll
-                for (int w = 0; w < 4; ++w) cls = min(cls, point_class(rec[4 * g + w], tab));
-            }
-            const uint32_t v = (cls == c) ? 1u : 0u;
-            uint32_t x = v;
+        for (int w = 0; w < 4; ++w) cls = min(cls, point_class(rec[4 * g + w], tab));
+        gcls[g] = (uint8_t)cls;
+        atomicAdd(&count[cls], 1u);
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        uint32_t run = 0;
+        for (int c = 0; c < S2_NCLASS; ++c) { cls_start[c] = run; carry[c] = 0; run += count[c]; }
+        cls_start[S2_NCLASS] = run;
+    }
+    __syncthreads();
+    // pass 2: stable position of every group inside its class, record written at the sorted place
+    for (int base = 0; base < n_groups; base += blockDim.x) {
+        const int g = base + threadIdx.x;
+        const int cls = (g < n_groups) ? (int)gcls[g] : S2_CLS_NONE;
+        uint32_t rank = 0;
 #pragma unroll
-            for (int d = 1; d < 32; d <<= 1) { uint32_t y = __shfl_up_sync(0xffffffffu, x, d); if (lane >= d) x += y; }
-            if (lane == 31) warp_sum[wid] = x;
-            __syncthreads();
-            if (wid == 0) {
-                uint32_t sv = (lane < nw) ? warp_sum[lane] : 0;
-#pragma unroll
-                for (int d = 1; d < 32; d <<= 1) { uint32_t y = __shfl_up_sync(0xffffffffu, sv, d); if (lane >= d) sv += y; }
-                warp_sum[lane] = sv;
-            }
-            __syncthreads();
-            const uint32_t pos = carry + (wid ? warp_sum[wid - 1] : 0) + (x - v);
-            if (v) {
-                GroupRec o;
-                o.g_orig = (uint32_t)g; o.cls = (uint32_t)c; o.pad0 = o.pad1 = 0;
-#pragma unroll
-                for (int w = 0; w < 4; ++w) {
-                    const PointRec r = rec[4 * g + w];
-#pragma unroll
-                    for (int i = 0; i < 5; ++i) o.T[i][w] = ((uint32_t)i < r.len) ? tab[r.off + i] : 0xFFFFFFFFu;
-#pragma unroll
-                    for (int b = 0; b < 4; ++b) o.f[w][b] = r.f[b];
-                }
-                grp[pos] = o;
-            }
-            __syncthreads();
-            if (threadIdx.x == blockDim.x - 1) carry = pos + v;
-            __syncthreads();
+        for (int k = 0; k < S2_NCLASS; ++k) {
+            const uint32_t bal = __ballot_sync(0xffffffffu, cls == k);
+            if (cls == k) rank = __popc(bal & ((1u << lane) - 1u));
+            if (lane == 0) wcnt[wid][k] = __popc(bal);
         }
-        if (threadIdx.x == 0) cls_start[c + 1] = carry;
+        __syncthreads();
+        if (threadIdx.x < S2_NCLASS) {
+            const int k = threadIdx.x;
+            uint32_t run = carry[k];
+            for (int w = 0; w < nw; ++w) { const uint32_t t = wcnt[w][k]; wcnt[w][k] = run; run += t; }
+            carry[k] = run;
+        }
+        __syncthreads();
+        if (cls < S2_NCLASS) {
+            const uint32_t pos = cls_start[cls] + wcnt[wid][cls] + rank;
+            GroupRec o;
+            o.g_orig = (uint32_t)g; o.cls = (uint32_t)cls; o.pad0 = o.pad1 = 0;
+#pragma unroll
+            for (int w = 0; w < 4; ++w) {
+                const PointRec r = rec[4 * g + w];
+#pragma unroll
+                for (int i = 0; i < 5; ++i) o.T[i][w] = ((uint32_t)i < r.len) ? tab[r.off + i] : 0xFFFFFFFFu;
+                if (cls <= S2_CLS_D5) o.T[4][w] = r.k0;     // the search classes keep k0 here
+#pragma unroll
+                for (int b = 0; b < 4; ++b) o.f[w][b] = r.f[b];
+            }
+            grp[pos] = o;
+        }
         __syncthreads();
     }
     if (threadIdx.x == 0) {
-        // segments: each class gets a share of seg_budget proportional to its estimated cost
-        const float wgt[S2_NCLASS] = {3.0f, 1.5f, 1.15f, 1.0f};
-        float total = 0.f;
-        for (int c = 0; c < S2_NCLASS; ++c) total += wgt[c] * (float)(cls_start[c + 1] - cls_start[c]);
         SegTable t;
-        t.n_seg = 0; t.pad = 0;
+        // padded search tables: D9 first, then D7, D5; a class that does not fit the arena is
+        // demoted to class 0 (the classes are adjacent in the sorted order, so this is a relabel)
+        const int64_t stride[4] = {0, 4 << 9, 4 << 7, 4 << 5};
+        int first_d = S2_CLS_D9;
+        for (;;) {
+            int64_t need = 0;
+            for (int c = first_d; c <= S2_CLS_D5; ++c) need += stride[c] * (int64_t)count[c];
+            if (need <= arena_cap || first_d > S2_CLS_D5) break;
+            first_d++;
+        }
+        int64_t off = 0;
         for (int c = 0; c < S2_NCLASS; ++c) {
-            const int n = (int)(cls_start[c + 1] - cls_start[c]);
+            t.cls_start[c] = (int32_t)cls_start[c];
+            t.arena_off[c] = 0;
+            if (c >= first_d && c <= S2_CLS_D5) { t.arena_off[c] = off; off += stride[c] * (int64_t)count[c]; }
+        }
+        t.cls_start[S2_NCLASS] = (int32_t)cls_start[S2_NCLASS];
+        t.first_d = first_d;
+        // segments: each class gets a share of seg_budget proportional to its estimated cost
+        const float wgt[S2_NCLASS] = {8.0f, 3.2f, 2.6f, 2.0f, 1.5f, 1.15f, 1.0f};
+        float total = 0.f;
+        for (int c = 0; c < S2_NCLASS; ++c) {
+            const float wc = (c >= 1 && c < first_d) ? wgt[0] : wgt[c];
+            total += wc * (float)count[c];
+        }
+        t.n_seg = 0;
+        for (int c = 0; c < S2_NCLASS; ++c) {
+            const int n = (int)count[c];
             if (n == 0) continue;
-            int k = (int)(wgt[c] * (float)n / total * (float)seg_budget + 0.5f);
-            k = max(1, min(k, min(n, S2_SEG_MAX - S2_NCLASS)));
+            const float wc = (c >= 1 && c < first_d) ? wgt[0] : wgt[c];
+            int k = (int)(wc * (float)n / total * (float)seg_budget + 0.5f);
+            k = max(1, min(k, n));
             for (int i = 0; i < k && t.n_seg < S2_SEG_MAX; ++i) {
                 t.g_lo[t.n_seg] = (int)cls_start[c] + (int)((int64_t)n * i / k);
                 t.g_hi[t.n_seg] = (int)cls_start[c] + (int)((int64_t)n * (i + 1) / k);
-                t.cls[t.n_seg] = c;
+                t.cls[t.n_seg] = (c >= 1 && c < first_d) ? 0 : c;
                 t.n_seg++;
             }
         }
         for (int i = t.n_seg; i < S2_SEG_MAX; ++i) { t.g_lo[i] = t.g_hi[i] = 0; t.cls[i] = 0; }
         seg_all[m] = t;
+    }
+}
+
+// Padded search tables of the D classes, one warp per sorted group: for each of its four points
+// 2^D words, the stored thresholds (minus 1) followed by 0xFFFFFFFF.
+__global__ void __launch_bounds__(256) k_fill_arena(const PointRec *__restrict__ rec_all,
+                                                    const uint32_t *__restrict__ tab_all, int64_t cap, int Jpad,
+                                                    const GroupRec *__restrict__ grp_all,
+                                                    const SegTable *__restrict__ seg_all,
+                                                    uint32_t *__restrict__ arena_all, int64_t arena_cap) {
+    const int m = blockIdx.y, n_groups = Jpad >> 2;
+    const SegTable *t = seg_all + m;
+    const int lane = threadIdx.x & 31;
+    const int first = t->cls_start[t->first_d <= S2_CLS_D5 ? t->first_d : S2_CLS_D5 + 1];
+    const int last = t->cls_start[S2_CLS_D5 + 1];
+    const PointRec *rec = rec_all + (size_t)m * Jpad;
+    const uint32_t *tab = tab_all + (size_t)m * cap;
+    uint32_t *arena = arena_all + (size_t)m * arena_cap;
+    for (int pos = first + blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5); pos < last;
+         pos += gridDim.x * (blockDim.x >> 5)) {
+        const GroupRec *g = grp_all + (size_t)m * n_groups + pos;
+        const int cls = (int)g->cls;
+        const int D = cls == S2_CLS_D9 ? 9 : (cls == S2_CLS_D7 ? 7 : 5);
+        uint32_t *dst = arena + t->arena_off[cls] + (int64_t)(pos - t->cls_start[cls]) * (4 << D);
+#pragma unroll
+        for (int w = 0; w < 4; ++w) {
+            const PointRec r = rec[g->g_orig * 4u + w];
+            for (int i = lane; i < (1 << D); i += 32) dst[(w << D) + i] = ((uint32_t)i < r.len) ? tab[r.off + i] : 0xFFFFFFFFu;
+        }
     }
 }
 
@@ -316,8 +384,11 @@ int pcmd_launch_stage1(pcmd_ctx *c, int n_models, cudaStream_t s) {
     int rc = build_tables(c, c->d_lambda, c->J, n_models, c->d_rawcnt, c->d_klo, c->d_q, c->cap_raw,
                           c->d_stcnt, c->d_tab, c->d_rec, c->Jpad, s);
     if (rc) return rc;
-    k_group_sort<<<n_models, 1024, 0, s>>>(c->d_rec, c->d_tab, c->cap_raw, c->Jpad, c->seg_budget, c->d_grp,
-                                           c->d_seg);
+    k_group_sort<<<n_models, 1024, 0, s>>>(c->d_rec, c->d_tab, c->cap_raw, c->Jpad, c->seg_budget, c->arena_cap,
+                                           c->d_gcls, c->d_grp, c->d_seg);
+    PCMD_LAUNCHED(c);
+    k_fill_arena<<<dim3(64, n_models), 256, 0, s>>>(c->d_rec, c->d_tab, c->cap_raw, c->Jpad, c->d_grp, c->d_seg,
+                                                     c->d_arena, c->arena_cap);
     PCMD_LAUNCHED(c);
     return PCMD_OK;
 }

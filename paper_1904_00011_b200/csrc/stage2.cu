@@ -17,6 +17,7 @@
 #define S2_TILE (S2_THREADS * S2_PX)
 #define S2_CHUNK 32          // groups per staged chunk (32 * 160 B = 5 KB)
 #define S2_FLUSH 16          // groups between flushes of the fp32 partial sums into fp64
+#define S2_TABW 4096         // words of staged search tables per buffer (16 KB): 32 / 8 / 2 groups of D5 / D7 / D9
 
 struct S2Args {
     const GroupRec *grp;     // [n_models][n_groups] class-sorted
@@ -24,7 +25,8 @@ struct S2Args {
     const PointRec *rec;     // [n_models][Jpad]  (generic class and overflow fix-up: k0, len, off)
     const uint32_t *tab;     // [n_models][cap]
     const uint64_t *mult;    // [Jpad]
-    int64_t cap;
+    const uint32_t *arena;   // [n_models][arena_cap] padded search tables of the D classes
+    int64_t cap, arena_cap;
     int Jpad, n_groups, B, n_models, n_tiles, seg_cap;
     int64_t P;
     uint32_t key0, key1, model0;
@@ -197,10 +199,34 @@ __device__ __forceinline__ void group_generic(S2State<NB, COUNTS> &st, const Gro
     }
 }
 
+// Classes D5/D7/D9: branch-free lower bound in the point's padded table (2^D words, staged in shared
+// memory): pos = #{stored thresholds below u}; every probe of a warp hits one table.
+template <int NB, bool COUNTS, int D>
+__device__ __forceinline__ void group_search(S2State<NB, COUNTS> &st, const GroupRec *__restrict__ g,
+                                             const uint32_t (&u)[S2_PX][4], const uint32_t *__restrict__ xt,
+                                             const uint64_t *__restrict__ mult) {
+#pragma unroll
+    for (int w = 0; w < 4; ++w) {
+        const float4 f = *reinterpret_cast<const float4 *>(g->f[w]);
+        const uint32_t k0 = g->T[4][w];
+        const uint32_t *X = xt + (w << D);
+#pragma unroll
+        for (int i = 0; i < S2_PX; ++i) {
+            const uint32_t x = u[i][w];
+            uint32_t pos = 0;
+#pragma unroll
+            for (int sft = D - 1; sft >= 0; --sft)
+                if (x > X[pos + (1u << sft) - 1u]) pos += 1u << sft;
+            add_stars<NB, COUNTS>(st, i, k0 + pos, f, g->g_orig * 4u + w, mult);
+        }
+    }
+}
+
 // ---- the persistent kernel ----------------------------------------------------------------------
 template <int NB, bool COUNTS>
 __global__ void __launch_bounds__(S2_THREADS) k_stage2(const S2Args a) {
     __shared__ __align__(128) GroupRec sbuf[2][S2_CHUNK];
+    __shared__ __align__(128) uint32_t stab[2][S2_TABW];
     __shared__ __align__(8) uint64_t bar[2];
     __shared__ int s_unit;
     if (threadIdx.x == 0) {
@@ -233,23 +259,27 @@ __global__ void __launch_bounds__(S2_THREADS) k_stage2(const S2Args a) {
 #pragma unroll
         for (int i = 0; i < S2_PX; ++i) pix[i] = (uint32_t)tile * S2_TILE + (uint32_t)i * S2_THREADS + threadIdx.x;
         st.reset();
-        const int n_chunks = (g_hi - g_lo + S2_CHUNK - 1) / S2_CHUNK;
-        if (threadIdx.x == 0 && n_chunks > 0) {
-            const uint32_t bytes = (uint32_t)min(S2_CHUNK, g_hi - g_lo) * (uint32_t)sizeof(GroupRec);
-            mbar_expect_tx(&bar[0], bytes);
-            bulk_g2s(sbuf[0], grp + g_lo, bytes, &bar[0]);
-        }
+        const int D = cls == S2_CLS_D9 ? 9 : (cls == S2_CLS_D7 ? 7 : (cls == S2_CLS_D5 ? 5 : 0));
+        const int csz = D ? (S2_TABW >> (D + 2)) : S2_CHUNK;       // groups per chunk
+        const uint32_t *xsrc = a.arena + (size_t)m * a.arena_cap + seg->arena_off[cls];
+        const int cls0 = seg->cls_start[cls];
+        const int n_chunks = (g_hi - g_lo + csz - 1) / csz;
+        auto stage = [&](int c, int buf) {      // thread 0: bulk copies of chunk c into buffer buf
+            const int g0 = g_lo + c * csz;
+            const uint32_t ng = (uint32_t)min(csz, g_hi - g0);
+            const uint32_t rbytes = ng * (uint32_t)sizeof(GroupRec), tbytes = D ? (ng << (D + 4)) : 0u;
+            mbar_expect_tx(&bar[buf], rbytes + tbytes);
+            bulk_g2s(sbuf[buf], grp + g0, rbytes, &bar[buf]);
+            if (D) bulk_g2s(stab[buf], xsrc + ((size_t)(g0 - cls0) << (D + 2)), tbytes, &bar[buf]);
+        };
+        if (threadIdx.x == 0 && n_chunks > 0) stage(0, 0);
         for (int c = 0; c < n_chunks; ++c) {
             const int cur = c & 1;
-            if (threadIdx.x == 0 && c + 1 < n_chunks) {   // prefetch the next chunk into the other buffer
-                const int g0 = g_lo + (c + 1) * S2_CHUNK;
-                const uint32_t bytes = (uint32_t)min(S2_CHUNK, g_hi - g0) * (uint32_t)sizeof(GroupRec);
-                mbar_expect_tx(&bar[cur ^ 1], bytes);
-                bulk_g2s(sbuf[cur ^ 1], grp + g0, bytes, &bar[cur ^ 1]);
-            }
+            if (threadIdx.x == 0 && c + 1 < n_chunks) stage(c + 1, cur ^ 1);   // prefetch
             if (cur == 0) { mbar_wait(&bar[0], phase0); phase0 ^= 1; }
             else { mbar_wait(&bar[1], phase1); phase1 ^= 1; }
-            const int ng = min(S2_CHUNK, g_hi - (g_lo + c * S2_CHUNK));
+            const int ng = min(csz, g_hi - (g_lo + c * csz));
+            const uint32_t *xt = stab[cur];
             const GroupRec *sb = sbuf[cur];
 #define S2_LOOP(BODY)                                                                          \
             for (int g = 0; g < ng; ++g) {                                                     \
@@ -261,9 +291,12 @@ __global__ void __launch_bounds__(S2_THREADS) k_stage2(const S2Args a) {
                 BODY;                                                                          \
                 if ((g & (S2_FLUSH - 1)) == S2_FLUSH - 1) st.flush();                          \
             }
-            if (cls == 3) { S2_LOOP((group_short<NB, COUNTS, 1>(st, gr, u, rec, tab, a.mult))) }
-            else if (cls == 2) { S2_LOOP((group_short<NB, COUNTS, 2>(st, gr, u, rec, tab, a.mult))) }
-            else if (cls == 1) { S2_LOOP((group_four<NB, COUNTS>(st, gr, u, rec, tab, a.mult))) }
+            if (cls == S2_CLS_L1) { S2_LOOP((group_short<NB, COUNTS, 1>(st, gr, u, rec, tab, a.mult))) }
+            else if (cls == S2_CLS_L2) { S2_LOOP((group_short<NB, COUNTS, 2>(st, gr, u, rec, tab, a.mult))) }
+            else if (cls == S2_CLS_L4) { S2_LOOP((group_four<NB, COUNTS>(st, gr, u, rec, tab, a.mult))) }
+            else if (cls == S2_CLS_D5) { S2_LOOP((group_search<NB, COUNTS, 5>(st, gr, u, xt + (g << 7), a.mult))) }
+            else if (cls == S2_CLS_D7) { S2_LOOP((group_search<NB, COUNTS, 7>(st, gr, u, xt + (g << 9), a.mult))) }
+            else if (cls == S2_CLS_D9) { S2_LOOP((group_search<NB, COUNTS, 9>(st, gr, u, xt + (g << 11), a.mult))) }
             else { S2_LOOP((group_generic<NB, COUNTS>(st, gr, u, rec, tab, a.mult))) }
 #undef S2_LOOP
             st.flush();
@@ -346,6 +379,7 @@ int pcmd_launch_stage2(pcmd_ctx *c, int n_models, uint64_t seed, uint32_t model0
                        uint64_t *d_hash, uint32_t *d_total, cudaStream_t s) {
     S2Args a;
     a.grp = c->d_grp; a.seg = c->d_seg; a.rec = c->d_rec; a.tab = c->d_tab; a.mult = c->d_mult;
+    a.arena = c->d_arena; a.arena_cap = c->arena_cap;
     a.cap = c->cap_raw; a.Jpad = c->Jpad; a.n_groups = c->Jpad >> 2; a.B = c->B; a.n_models = n_models;
     a.n_tiles = (int)((c->P + S2_TILE - 1) / S2_TILE); a.seg_cap = c->seg_cap; a.P = c->P;
     a.key0 = (uint32_t)(seed & 0xFFFFFFFFull); a.key1 = (uint32_t)(seed >> 32); a.model0 = model0;
