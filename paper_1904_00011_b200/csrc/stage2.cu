@@ -12,8 +12,15 @@
 // segment order.
 #include "pcmd_internal.cuh"
 
+#ifndef S2_THREADS
 #define S2_THREADS 256
+#endif
+#ifndef S2_PX
 #define S2_PX 2
+#endif
+#ifndef S2_MINB
+#define S2_MINB 1
+#endif
 #define S2_TILE (S2_THREADS * S2_PX)
 #define S2_CHUNK 32          // groups per staged chunk (32 * 160 B = 5 KB)
 #define S2_FLUSH 16          // groups between flushes of the fp32 partial sums into fp64
@@ -201,30 +208,36 @@ __device__ __forceinline__ void group_generic(S2State<NB, COUNTS> &st, const Gro
 
 // Classes D5/D7/D9: branch-free lower bound in the point's padded table (2^D words, staged in shared
 // memory): pos = #{stored thresholds below u}; every probe of a warp hits one table.
+// xbuf: the staged table buffer; xoff: byte offset of this group's four tables inside it.
 template <int NB, bool COUNTS, int D>
 __device__ __forceinline__ void group_search(S2State<NB, COUNTS> &st, const GroupRec *__restrict__ g,
-                                             const uint32_t (&u)[S2_PX][4], const uint32_t *__restrict__ xt,
-                                             const uint64_t *__restrict__ mult) {
+                                             const uint32_t (&u)[S2_PX][4], const uint32_t *__restrict__ xbuf,
+                                             uint32_t xoff, const uint64_t *__restrict__ mult) {
+    const char *X = reinterpret_cast<const char *>(xbuf);
 #pragma unroll
     for (int w = 0; w < 4; ++w) {
         const float4 f = *reinterpret_cast<const float4 *>(g->f[w]);
-        const uint32_t k0 = g->T[4][w];
-        const uint32_t *X = xt + (w << D);
+        const uint32_t lo = xoff + ((uint32_t)w << (D + 2)), hi = lo + (2u << D);   // byte offsets of X[0], X[2^(D-1)]
+        const uint32_t kb = g->T[4][w] - (lo >> 2);                                 // k0 - lo/4 (mod 2^32)
+        const uint32_t t0 = *reinterpret_cast<const uint32_t *>(X + hi - 4u);       // first probe: warp-uniform
 #pragma unroll
         for (int i = 0; i < S2_PX; ++i) {
             const uint32_t x = u[i][w];
-            uint32_t pos = 0;
+            uint32_t off = (x > t0) ? hi : lo;                                      // byte offset of X[pos]
 #pragma unroll
-            for (int sft = D - 1; sft >= 0; --sft)
-                if (x > X[pos + (1u << sft) - 1u]) pos += 1u << sft;
-            add_stars<NB, COUNTS>(st, i, k0 + pos, f, g->g_orig * 4u + w, mult);
+            for (int sft = D - 2; sft >= 0; --sft) {
+                const uint32_t t = *reinterpret_cast<const uint32_t *>(X + off + ((4u << sft) - 4u));
+                asm("{\n.reg .pred p;\nsetp.gt.u32 p, %1, %2;\n@p add.u32 %0, %0, %3;\n}"
+                    : "+r"(off) : "r"(x), "r"(t), "r"(4u << sft));
+            }
+            add_stars<NB, COUNTS>(st, i, (off >> 2) + kb, f, g->g_orig * 4u + w, mult);
         }
     }
 }
 
 // ---- the persistent kernel ----------------------------------------------------------------------
 template <int NB, bool COUNTS>
-__global__ void __launch_bounds__(S2_THREADS) k_stage2(const S2Args a) {
+__global__ void __launch_bounds__(S2_THREADS, S2_MINB) k_stage2(const S2Args a) {
     __shared__ __align__(128) GroupRec sbuf[2][S2_CHUNK];
     __shared__ __align__(128) uint32_t stab[2][S2_TABW];
     __shared__ __align__(8) uint64_t bar[2];
@@ -235,8 +248,7 @@ __global__ void __launch_bounds__(S2_THREADS) k_stage2(const S2Args a) {
     }
     __syncthreads();
     uint32_t phase0 = 0, phase1 = 0;                 // parity of the next completion of each barrier
-    const int units_per_model = a.n_tiles * a.seg_cap;
-    const int n_units = a.n_models * units_per_model;
+    const int n_units = a.n_models * a.n_tiles * a.seg_cap;
     S2State<NB, COUNTS> st;
     for (;;) {
         if (threadIdx.x == 0) s_unit = atomicAdd(a.counter, 1);
@@ -244,9 +256,10 @@ __global__ void __launch_bounds__(S2_THREADS) k_stage2(const S2Args a) {
         const int unit = s_unit;
         __syncthreads();
         if (unit >= n_units) break;
-        // segment-major order: the expensive classes (low segment numbers) are handed out first
-        const int sg = unit / (a.n_models * a.n_tiles);
-        const int rem = unit - sg * (a.n_models * a.n_tiles);
+        // segment-minor order: consecutive units are different segments (classes) of one tile, so the
+        // CTAs resident on an SM mix multiply-bound (L) and compare-bound (D) classes
+        const int sg = unit % a.seg_cap;
+        const int rem = unit / a.seg_cap;
         const int m = rem / a.n_tiles, tile = rem - m * a.n_tiles;
         const SegTable *seg = a.seg + m;
         if (sg >= seg->n_seg) continue;
@@ -264,7 +277,7 @@ __global__ void __launch_bounds__(S2_THREADS) k_stage2(const S2Args a) {
         const uint32_t *xsrc = a.arena + (size_t)m * a.arena_cap + seg->arena_off[cls];
         const int cls0 = seg->cls_start[cls];
         const int n_chunks = (g_hi - g_lo + csz - 1) / csz;
-        auto stage = [&](int c, int buf) {      // thread 0: bulk copies of chunk c into buffer buf
+        auto stage = [&](int c, int buf) {      // thread 0: bulk copies (TMA) of chunk c into buffer buf
             const int g0 = g_lo + c * csz;
             const uint32_t ng = (uint32_t)min(csz, g_hi - g0);
             const uint32_t rbytes = ng * (uint32_t)sizeof(GroupRec), tbytes = D ? (ng << (D + 4)) : 0u;
@@ -294,13 +307,13 @@ __global__ void __launch_bounds__(S2_THREADS) k_stage2(const S2Args a) {
             if (cls == S2_CLS_L1) { S2_LOOP((group_short<NB, COUNTS, 1>(st, gr, u, rec, tab, a.mult))) }
             else if (cls == S2_CLS_L2) { S2_LOOP((group_short<NB, COUNTS, 2>(st, gr, u, rec, tab, a.mult))) }
             else if (cls == S2_CLS_L4) { S2_LOOP((group_four<NB, COUNTS>(st, gr, u, rec, tab, a.mult))) }
-            else if (cls == S2_CLS_D5) { S2_LOOP((group_search<NB, COUNTS, 5>(st, gr, u, xt + (g << 7), a.mult))) }
-            else if (cls == S2_CLS_D7) { S2_LOOP((group_search<NB, COUNTS, 7>(st, gr, u, xt + (g << 9), a.mult))) }
-            else if (cls == S2_CLS_D9) { S2_LOOP((group_search<NB, COUNTS, 9>(st, gr, u, xt + (g << 11), a.mult))) }
+            else if (cls == S2_CLS_D5) { S2_LOOP((group_search<NB, COUNTS, 5>(st, gr, u, xt, (uint32_t)g << 9, a.mult))) }
+            else if (cls == S2_CLS_D7) { S2_LOOP((group_search<NB, COUNTS, 7>(st, gr, u, xt, (uint32_t)g << 11, a.mult))) }
+            else if (cls == S2_CLS_D9) { S2_LOOP((group_search<NB, COUNTS, 9>(st, gr, u, xt, (uint32_t)g << 13, a.mult))) }
             else { S2_LOOP((group_generic<NB, COUNTS>(st, gr, u, rec, tab, a.mult))) }
 #undef S2_LOOP
             st.flush();
-            __syncthreads();   // every warp is done with sbuf[cur] before it is refilled
+            __syncthreads();   // every warp is done with the buffers of chunk c before they are refilled
         }
         // partial flux of this (segment, tile); exact integer counts by atomics (parity build)
 #pragma unroll
