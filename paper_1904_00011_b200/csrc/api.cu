@@ -36,8 +36,8 @@ static void free_scratch(pcmd_ctx *c) {
     cudaFree(c->d_sfh); cudaFree(c->d_model); cudaFree(c->d_mdfw); cudaFree(c->d_lambda);
     cudaFree(c->d_rawcnt); cudaFree(c->d_klo); cudaFree(c->d_q); cudaFree(c->d_stcnt);
     cudaFree(c->d_tab); cudaFree(c->d_rec); cudaFree(c->d_fdust); cudaFree(c->d_grp); cudaFree(c->d_seg);
-    cudaFree(c->d_gcls); cudaFree(c->d_arena);
-    c->d_grp = nullptr; c->d_seg = nullptr; c->d_gcls = nullptr; c->d_arena = nullptr;
+    cudaFree(c->d_gcls); cudaFree(c->d_arena); cudaFree(c->d_gpos);
+    c->d_grp = nullptr; c->d_seg = nullptr; c->d_gcls = nullptr; c->d_arena = nullptr; c->d_gpos = nullptr;
     if (c->h_stage) cudaFreeHost(c->h_stage);
     c->d_sfh = nullptr; c->d_model = nullptr; c->d_mdfw = nullptr; c->d_lambda = nullptr;
     c->d_rawcnt = nullptr; c->d_klo = nullptr; c->d_q = nullptr; c->d_stcnt = nullptr;
@@ -67,6 +67,7 @@ static int ensure_scratch(pcmd_ctx *c, int n_models, int64_t cap_raw) {
     PCMD_CUDA(c, cudaMalloc(&c->d_grp, (size_t)nm * (Jp / 4) * sizeof(GroupRec)));
     PCMD_CUDA(c, cudaMalloc(&c->d_seg, (size_t)nm * sizeof(SegTable)));
     PCMD_CUDA(c, cudaMalloc(&c->d_gcls, (size_t)nm * (Jp / 4)));
+    PCMD_CUDA(c, cudaMalloc(&c->d_gpos, (size_t)nm * (Jp / 4) * sizeof(uint32_t)));
     {   // padded search tables: room for every group in D9 (8 KB), capped at 1 GiB over all models
         int64_t words = (int64_t)(Jp / 4) * 2048, lim = ((int64_t)1 << 28) / nm;
         if (words > lim) words = lim;

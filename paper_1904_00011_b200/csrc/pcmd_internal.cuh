@@ -84,6 +84,7 @@ struct pcmd_ctx {
     GroupRec *d_grp;       // [cap_models][Jpad/4] class-sorted group records
     SegTable *d_seg;       // [cap_models]
     uint8_t *d_gcls;       // [cap_models][Jpad/4] class of each group (original order)
+    uint32_t *d_gpos;      // [cap_models][Jpad/4] sorted position of each group
     uint32_t *d_arena; int64_t arena_cap;  // [cap_models][arena_cap] padded search tables of the D classes
     float *d_part;  int64_t part_elems;  // stage-2 partial fluxes [cap_models][seg_cap][B][P]
     int32_t seg_budget, seg_cap, s2_ctas_per_sm;

@@ -21,9 +21,9 @@ __device__ double expneg_basic(double t) {
     return p;
 }
 
-// grid = n_models.  Thread 0 computes the MDF weights in the stated order; all threads then
-// compute lambda_j and the per-star fluxes.
-__global__ void k_weights(const DevModel *__restrict__ mdl, const double *__restrict__ sfh,
+// grid = (blocks over points, n_models).  Thread 0 of every block computes the MDF weights in the
+// stated order (Z values; block 0 stores them); all threads then compute lambda_j and the fluxes.
+__global__ void __launch_bounds__(256) k_weights(const DevModel *__restrict__ mdl, const double *__restrict__ sfh,
                           const double *__restrict__ feh_grid, const int32_t *__restrict__ age_idx,
                           const int32_t *__restrict__ feh_idx, const double *__restrict__ imf_w,
                           const double *__restrict__ absmag, int A, int Z, int J, int Jpad, int B,
@@ -31,7 +31,7 @@ __global__ void k_weights(const DevModel *__restrict__ mdl, const double *__rest
                           double *__restrict__ mdfw_out, double *__restrict__ lambda_out,
                           PointRec *__restrict__ rec_out, int32_t *status) {
     extern __shared__ double w[];  // [Z]
-    const int m = blockIdx.x;
+    const int m = blockIdx.y;
     const DevModel M = mdl[m];
     if (threadIdx.x == 0) {
         double e_min = INFINITY;
@@ -48,23 +48,26 @@ __global__ void k_weights(const DevModel *__restrict__ mdl, const double *__rest
             if (w[z] < mdf_cut) w[z] = 0.0;
             G2 = __dadd_rn(G2, w[z]);
         }
-        for (int z = 0; z < Z; ++z) { w[z] = __ddiv_rn(w[z], G2); mdfw_out[(size_t)m * Z + z] = w[z]; }
+        for (int z = 0; z < Z; ++z) {
+            w[z] = __ddiv_rn(w[z], G2);
+            if (blockIdx.x == 0) mdfw_out[(size_t)m * Z + z] = w[z];
+        }
     }
     __syncthreads();
     const double zp[4] = {zp0, zp1, zp2, zp3};
-    for (int j = threadIdx.x; j < Jpad; j += blockDim.x) {
-        PointRec r;
-        r.T0 = 0xFFFFFFFFu; r.off = 0; r.len = 0; r.k0 = 0;
-        r.f[0] = r.f[1] = r.f[2] = r.f[3] = 0.f;
-        if (j < J) {
-            double lam = __dmul_rn(__dmul_rn(sfh[(size_t)m * A + age_idx[j]], w[feh_idx[j]]), imf_w[j]);
-            lambda_out[(size_t)m * J + j] = lam;
-            if (!(lam >= 0.0) || lam > PCMD_LAMBDA_MAX) atomicMin(status, PCMD_ERANGE);
-            for (int b = 0; b < B; ++b)  // fluxes according to the distance
-                r.f[b] = (float)pow(10.0, -0.4 * (absmag[(size_t)j * B + b] + M.dmod - zp[b]));
-        }
-        rec_out[(size_t)m * Jpad + j] = r;
+    const int j = blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= Jpad) return;
+    PointRec r;
+    r.T0 = 0xFFFFFFFFu; r.off = 0; r.len = 0; r.k0 = 0;
+    r.f[0] = r.f[1] = r.f[2] = r.f[3] = 0.f;
+    if (j < J) {
+        double lam = __dmul_rn(__dmul_rn(sfh[(size_t)m * A + age_idx[j]], w[feh_idx[j]]), imf_w[j]);
+        lambda_out[(size_t)m * J + j] = lam;
+        if (!(lam >= 0.0) || lam > PCMD_LAMBDA_MAX) atomicMin(status, PCMD_ERANGE);
+        for (int b = 0; b < B; ++b)  // fluxes according to the distance
+            r.f[b] = (float)exp10(-0.4 * (absmag[(size_t)j * B + b] + M.dmod - zp[b]));
     }
+    rec_out[(size_t)m * Jpad + j] = r;
 }
 
 // Range [k_lo, k_hi] of the relative pmf q[k] >= 2^-64 (R-C2 step 1), one thread per point.
@@ -202,7 +205,10 @@ __global__ void k_table_compact(int J, int n_models, const uint32_t *__restrict_
 // D5/D7/D9: table of at most 2^D - 1 thresholds, searched branch-free in shared memory;
 // class 0: longer tables, bisection in global memory.  A group takes the most expensive class
 // of its four points.
-#define S2_OVF_THR 4290772991u   /* 2^32 (1 - 2^-10) - 1 */
+#ifndef S2_OVF_LOG2
+#define S2_OVF_LOG2 10
+#endif
+#define S2_OVF_THR (0xFFFFFFFFu - (1u << (32 - S2_OVF_LOG2)))   /* 2^32 (1 - 2^-10) - 1 */
 
 __device__ __forceinline__ int point_class(const PointRec &r, const uint32_t *__restrict__ tab) {
     if (r.len == 0 && r.k0 == 0) return S2_CLS_NONE;      // never a star
@@ -217,29 +223,35 @@ __device__ __forceinline__ int point_class(const PointRec &r, const uint32_t *__
     return 0;
 }
 
-__global__ void __launch_bounds__(1024) k_group_sort(const PointRec *__restrict__ rec_all,
-                                                     const uint32_t *__restrict__ tab_all, int64_t cap,
-                                                     int Jpad, int seg_budget, int64_t arena_cap,
-                                                     uint8_t *__restrict__ cls_all, GroupRec *__restrict__ grp_all,
+// Class of every group: one thread per group.
+__global__ void __launch_bounds__(256) k_group_classify(const PointRec *__restrict__ rec_all,
+                                                        const uint32_t *__restrict__ tab_all, int64_t cap, int Jpad,
+                                                        uint8_t *__restrict__ cls_all) {
+    const int m = blockIdx.y, n_groups = Jpad >> 2;
+    const int g = blockIdx.x * blockDim.x + threadIdx.x;
+    if (g >= n_groups) return;
+    const PointRec *rec = rec_all + (size_t)m * Jpad;
+    const uint32_t *tab = tab_all + (size_t)m * cap;
+    int cls = S2_CLS_NONE;
+#pragma unroll
+    for (int w = 0; w < 4; ++w) cls = min(cls, point_class(rec[4 * g + w], tab));
+    cls_all[(size_t)m * n_groups + g] = (uint8_t)cls;
+}
+
+// Stable counting sort of the groups by class (positions only), segment table, arena layout.
+// One block per model.
+__global__ void __launch_bounds__(1024) k_group_sort(const uint8_t *__restrict__ cls_all, int Jpad, int seg_budget,
+                                                     int64_t arena_cap, uint32_t *__restrict__ pos_all,
                                                      SegTable *__restrict__ seg_all) {
     __shared__ uint32_t wcnt[32][S2_NCLASS];
     __shared__ uint32_t count[S2_NCLASS + 1], carry[S2_NCLASS], cls_start[S2_NCLASS + 1];
     const int m = blockIdx.x, n_groups = Jpad >> 2;
-    const PointRec *rec = rec_all + (size_t)m * Jpad;
-    const uint32_t *tab = tab_all + (size_t)m * cap;
-    GroupRec *grp = grp_all + (size_t)m * n_groups;
-    uint8_t *gcls = cls_all + (size_t)m * n_groups;
+    const uint8_t *gcls = cls_all + (size_t)m * n_groups;
+    uint32_t *gpos = pos_all + (size_t)m * n_groups;
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
     if (threadIdx.x <= S2_NCLASS) count[threadIdx.x] = 0;
     __syncthreads();
-    // pass 1: class of every group, class populations
-    for (int g = threadIdx.x; g < n_groups; g += blockDim.x) {
-        int cls = S2_CLS_NONE;
-#pragma unroll
-        for (int w = 0; w < 4; ++w) cls = min(cls, point_class(rec[4 * g + w], tab));
-        gcls[g] = (uint8_t)cls;
-        atomicAdd(&count[cls], 1u);
-    }
+    for (int g = threadIdx.x; g < n_groups; g += blockDim.x) atomicAdd(&count[gcls[g]], 1u);
     __syncthreads();
     if (threadIdx.x == 0) {
         uint32_t run = 0;
@@ -247,7 +259,6 @@ __global__ void __launch_bounds__(1024) k_group_sort(const PointRec *__restrict_
         cls_start[S2_NCLASS] = run;
     }
     __syncthreads();
-    // pass 2: stable position of every group inside its class, record written at the sorted place
     for (int base = 0; base < n_groups; base += blockDim.x) {
         const int g = base + threadIdx.x;
         const int cls = (g < n_groups) ? (int)gcls[g] : S2_CLS_NONE;
@@ -266,21 +277,7 @@ __global__ void __launch_bounds__(1024) k_group_sort(const PointRec *__restrict_
             carry[k] = run;
         }
         __syncthreads();
-        if (cls < S2_NCLASS) {
-            const uint32_t pos = cls_start[cls] + wcnt[wid][cls] + rank;
-            GroupRec o;
-            o.g_orig = (uint32_t)g; o.cls = (uint32_t)cls; o.pad0 = o.pad1 = 0;
-#pragma unroll
-            for (int w = 0; w < 4; ++w) {
-                const PointRec r = rec[4 * g + w];
-#pragma unroll
-                for (int i = 0; i < 5; ++i) o.T[i][w] = ((uint32_t)i < r.len) ? tab[r.off + i] : 0xFFFFFFFFu;
-                if (cls <= S2_CLS_D5) o.T[4][w] = r.k0;     // the search classes keep k0 here
-#pragma unroll
-                for (int b = 0; b < 4; ++b) o.f[w][b] = r.f[b];
-            }
-            grp[pos] = o;
-        }
+        if (g < n_groups) gpos[g] = (cls < S2_NCLASS) ? cls_start[cls] + wcnt[wid][cls] + rank : 0xFFFFFFFFu;
         __syncthreads();
     }
     if (threadIdx.x == 0) {
@@ -329,31 +326,43 @@ __global__ void __launch_bounds__(1024) k_group_sort(const PointRec *__restrict_
     }
 }
 
-// Padded search tables of the D classes, one warp per sorted group: for each of its four points
-// 2^D words, the stored thresholds (minus 1) followed by 0xFFFFFFFF.
-__global__ void __launch_bounds__(256) k_fill_arena(const PointRec *__restrict__ rec_all,
+// Group records at their sorted places and the padded search tables of the D classes: one warp
+// per group.  Lane w < 4 writes point w's part of the record; all lanes write the padded tables
+// (2^D words per point: the stored thresholds minus 1, then 0xFFFFFFFF).
+__global__ void __launch_bounds__(256) k_group_emit(const PointRec *__restrict__ rec_all,
                                                     const uint32_t *__restrict__ tab_all, int64_t cap, int Jpad,
-                                                    const GroupRec *__restrict__ grp_all,
-                                                    const SegTable *__restrict__ seg_all,
+                                                    const uint8_t *__restrict__ cls_all,
+                                                    const uint32_t *__restrict__ pos_all,
+                                                    const SegTable *__restrict__ seg_all, GroupRec *__restrict__ grp_all,
                                                     uint32_t *__restrict__ arena_all, int64_t arena_cap) {
-    const int m = blockIdx.y, n_groups = Jpad >> 2;
-    const SegTable *t = seg_all + m;
-    const int lane = threadIdx.x & 31;
-    const int first = t->cls_start[t->first_d <= S2_CLS_D5 ? t->first_d : S2_CLS_D5 + 1];
-    const int last = t->cls_start[S2_CLS_D5 + 1];
+    const int m = blockIdx.y, n_groups = Jpad >> 2, lane = threadIdx.x & 31;
+    const int g = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    if (g >= n_groups) return;
+    const int cls = (int)cls_all[(size_t)m * n_groups + g];
+    if (cls >= S2_NCLASS) return;
+    const uint32_t pos = pos_all[(size_t)m * n_groups + g];
     const PointRec *rec = rec_all + (size_t)m * Jpad;
     const uint32_t *tab = tab_all + (size_t)m * cap;
-    uint32_t *arena = arena_all + (size_t)m * arena_cap;
-    for (int pos = first + blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5); pos < last;
-         pos += gridDim.x * (blockDim.x >> 5)) {
-        const GroupRec *g = grp_all + (size_t)m * n_groups + pos;
-        const int cls = (int)g->cls;
+    GroupRec *o = grp_all + (size_t)m * n_groups + pos;
+    if (lane < 4) {
+        const int w = lane;
+        const PointRec r = rec[4 * g + w];
+        if (w == 0) { o->g_orig = (uint32_t)g; o->cls = (uint32_t)cls; o->pad0 = o->pad1 = 0; }
+#pragma unroll
+        for (int i = 0; i < 5; ++i) o->T[i][w] = ((uint32_t)i < r.len) ? tab[r.off + i] : 0xFFFFFFFFu;
+        if (cls <= S2_CLS_D5) o->T[4][w] = r.k0;     // the search classes keep k0 here
+#pragma unroll
+        for (int b = 0; b < 4; ++b) o->f[w][b] = r.f[b];
+    }
+    const SegTable *t = seg_all + m;
+    if (cls >= t->first_d && cls <= S2_CLS_D5) {
         const int D = cls == S2_CLS_D9 ? 9 : (cls == S2_CLS_D7 ? 7 : 5);
-        uint32_t *dst = arena + t->arena_off[cls] + (int64_t)(pos - t->cls_start[cls]) * (4 << D);
+        uint32_t *dst = arena_all + (size_t)m * arena_cap + t->arena_off[cls] +
+                        (int64_t)((int)pos - t->cls_start[cls]) * (4 << D);
 #pragma unroll
         for (int w = 0; w < 4; ++w) {
-            const PointRec r = rec[g->g_orig * 4u + w];
-            for (int i = lane; i < (1 << D); i += 32) dst[(w << D) + i] = ((uint32_t)i < r.len) ? tab[r.off + i] : 0xFFFFFFFFu;
+            const uint32_t off = rec[4 * g + w].off, len = rec[4 * g + w].len;
+            for (int i = lane; i < (1 << D); i += 32) dst[(w << D) + i] = ((uint32_t)i < len) ? tab[off + i] : 0xFFFFFFFFu;
         }
     }
 }
@@ -376,7 +385,7 @@ static int build_tables(pcmd_ctx *c, const double *d_lambda, int J, int n_models
 }
 
 int pcmd_launch_stage1(pcmd_ctx *c, int n_models, cudaStream_t s) {
-    k_weights<<<n_models, 256, c->Z * sizeof(double), s>>>(
+    k_weights<<<dim3((c->Jpad + 255) / 256, n_models), 256, c->Z * sizeof(double), s>>>(
         c->d_model, c->d_sfh, c->d_feh_grid, c->d_age_idx, c->d_feh_idx, c->d_imf_w, c->d_absmag, c->A,
         c->Z, c->J, c->Jpad, c->B, c->mdf_cut, c->zp[0], c->zp[1], c->zp[2], c->zp[3], c->d_mdfw,
         c->d_lambda, c->d_rec, c->d_status);
@@ -384,11 +393,15 @@ int pcmd_launch_stage1(pcmd_ctx *c, int n_models, cudaStream_t s) {
     int rc = build_tables(c, c->d_lambda, c->J, n_models, c->d_rawcnt, c->d_klo, c->d_q, c->cap_raw,
                           c->d_stcnt, c->d_tab, c->d_rec, c->Jpad, s);
     if (rc) return rc;
-    k_group_sort<<<n_models, 1024, 0, s>>>(c->d_rec, c->d_tab, c->cap_raw, c->Jpad, c->seg_budget, c->arena_cap,
-                                           c->d_gcls, c->d_grp, c->d_seg);
+    const int n_groups = c->Jpad >> 2;
+    k_group_classify<<<dim3((n_groups + 255) / 256, n_models), 256, 0, s>>>(c->d_rec, c->d_tab, c->cap_raw, c->Jpad,
+                                                                           c->d_gcls);
     PCMD_LAUNCHED(c);
-    k_fill_arena<<<dim3(64, n_models), 256, 0, s>>>(c->d_rec, c->d_tab, c->cap_raw, c->Jpad, c->d_grp, c->d_seg,
-                                                     c->d_arena, c->arena_cap);
+    k_group_sort<<<n_models, 1024, 0, s>>>(c->d_gcls, c->Jpad, c->seg_budget, c->arena_cap, c->d_gpos, c->d_seg);
+    PCMD_LAUNCHED(c);
+    k_group_emit<<<dim3((n_groups + 7) / 8, n_models), 256, 0, s>>>(c->d_rec, c->d_tab, c->cap_raw, c->Jpad, c->d_gcls,
+                                                                    c->d_gpos, c->d_seg, c->d_grp, c->d_arena,
+                                                                    c->arena_cap);
     PCMD_LAUNCHED(c);
     return PCMD_OK;
 }
