@@ -44,6 +44,9 @@ from workloads import synthetic as W  # noqa: E402
 METRIC = "pcmd_model_evals_per_s"
 UNIT = "evals/s"
 SM_COUNT, SCHED_PER_SM, LANES = 148, 4, 32
+# measured on this pool's B200 (profiles/README.md): a kernel that does nothing but Philox4x32-10
+# delivers 5.13e11 calls/s = 2.05e12 draws/s (the IMAD.WIDE pipe is the tightest pipe of stage 2)
+PHILOX_CEILING_DRAWS = 2.05e12
 
 
 def i_alg(n_bands: int) -> int:
@@ -219,8 +222,9 @@ def run_ours(args):
     torch.cuda.synchronize()
     if g.status() != 0:
         raise SystemExit("device status %d" % g.status())
-    lam = g.debug_weights(0)["lam"]
-    draws_per_model = int((lam > 0).sum()) * g.P
+    # draws of one step on this rank: P x #{j: lambda_j > 0}, summed over the batch's models
+    # (models with a narrow MDF have whole isochrones cut to lambda = 0: those are not drawn)
+    draws_step = sum(int((g.debug_weights(i)["lam"] > 0).sum()) for i in range(n)) * g.P
     g.profile(True)
 
     # ---- device-timed leg
@@ -272,7 +276,7 @@ def run_ours(args):
         ms_step = total_ms / args.steps
         evals = n * world * args.steps / (total_ms * 1e-3)
         s2_ms = float(stage[1]) / args.steps
-        draws = draws_per_model * n
+        draws = draws_step
         ia = i_alg(g.B)
         peak_inst = SM_COUNT * SCHED_PER_SM * LANES * float(peaks.get("sm_max_mhz", 1965.0)) * 1e6 / 1e12
         ach = draws * ia / (s2_ms * 1e-3) / 1e12 if s2_ms > 0 else 0.0
@@ -293,6 +297,7 @@ def run_ours(args):
                 "roofline": {"kernel": "k_stage2 (Poisson draws -> pixel flux)", "bound": "alu",
                              "achieved": ach, "peak": peak_inst, "unit": "Tinst/s",
                              "frac": ach / peak_inst, "traffic": None,
+                             "frac_of_philox_ceiling": (draws / (s2_ms * 1e-3)) / PHILOX_CEILING_DRAWS if s2_ms > 0 else None,
                              "i_alg_thread_inst_per_draw": ia, "draws_per_launch": draws,
                              "ms_per_launch": s2_ms, "peak_source": which + " sm_max_mhz"}}
         if world == 1 and not args.no_cpu:

@@ -152,6 +152,7 @@ extern "C" int pcmd_create(pcmd_ctx **out, const pcmd_config *cfg) {
         rc = upload(c, &c->d_psf, p2, (size_t)B * K * K);
         free(p2);
         if (rc) { pcmd_destroy(c); return rc; }
+        if (cfg->psf_separable) TRY(upload(c, &c->d_psf_sep, cfg->psf, (size_t)B * 2 * K));
     }
     {
         uint64_t *mult = (uint64_t *)malloc((size_t)c->Jpad * sizeof(uint64_t));
@@ -192,7 +193,7 @@ extern "C" void pcmd_destroy(pcmd_ctx *c) {
     cudaDeviceSynchronize();
     free_scratch(c);
     cudaFree(c->d_age_idx); cudaFree(c->d_feh_idx); cudaFree(c->d_imf_w); cudaFree(c->d_absmag);
-    cudaFree(c->d_feh_grid); cudaFree(c->d_psf); cudaFree(c->d_mult); cudaFree(c->d_hess_spec);
+    cudaFree(c->d_feh_grid); cudaFree(c->d_psf); cudaFree(c->d_psf_sep); cudaFree(c->d_mult); cudaFree(c->d_hess_spec);
     cudaFree(c->d_sky_tab); cudaFree(c->d_status); cudaFree(c->d_hpart); cudaFree(c->d_part);
     cudaFree(c->d_mag); cudaFree(c->d_hessbuf); cudaFree(c->d_statbuf); cudaFree(c->d_lnl);
     cudaFree(c->d_hess_data); cudaFree(c->d_data_stats);

@@ -10,6 +10,7 @@
 struct CvArgs {
     const float *F;      // [n_models][B][P] dusty flux
     const float *psf;    // [B][K][K]
+    const float *psf_sep; // [B][2][K] row factor, column factor (separable PSFs only)
     float *mag;          // [n_models][B][P]
     float *tap_conv;     // optional
     const uint32_t *sky_tab;
@@ -20,6 +21,9 @@ struct CvArgs {
     uint32_t key0, key1, model0;
     double zp[4], sky[4], read_sigma[4];
 };
+
+__device__ __forceinline__ void noise_mag_epilogue(const CvArgs &a, const float (&acc)[CV_TY / CV_ROWS], int x0, int y0,
+                                                   int lx, int m, int b, int mb);
 
 __global__ void __launch_bounds__(CV_TX * CV_ROWS) k_conv_noise(const CvArgs a) {
     extern __shared__ float sm[];
@@ -52,6 +56,55 @@ __global__ void __launch_bounds__(CV_TX * CV_ROWS) k_conv_noise(const CvArgs a) 
                 acc[q] = fmaf(w, tile[(ly + 2 * r - ka) * TW + (lx + 2 * r - kb)], acc[q]);
             }
         }
+    noise_mag_epilogue(a, acc, x0, y0, lx, m, b, mb);
+}
+
+// Separable PSF (column factor (x) row factor, R-Q10): row pass over the halo tile into shared
+// memory, then the column pass: 2K FMAs per output instead of K^2.  Same tile, halo and epilogue.
+__global__ void __launch_bounds__(CV_TX * CV_ROWS) k_conv_noise_sep(const CvArgs a) {
+    extern __shared__ float sm[];
+    const int K = a.K, r = (K - 1) / 2, N = a.N;
+    const int TW = CV_TX + K - 1, TH = CV_TY + K - 1;
+    float *tile = sm;                  // [TH][TW]
+    float *hrow = sm + TH * TW;        // [TH][CV_TX] row-convolved
+    float *fac = hrow + TH * CV_TX;    // [2][K]: row factor, column factor
+    const int mb = blockIdx.z, m = mb / a.B, b = mb - m * a.B;
+    const float *F = a.F + (size_t)mb * a.P;
+    const int x0 = blockIdx.x * CV_TX, y0 = blockIdx.y * CV_TY;
+    const int tid = threadIdx.y * CV_TX + threadIdx.x, nt = CV_TX * CV_ROWS;
+    for (int t = tid; t < 2 * K; t += nt) fac[t] = a.psf_sep[(size_t)b * 2 * K + t];
+    for (int t = tid; t < TH * TW; t += nt) {
+        int i = t / TW, j = t - i * TW;
+        int yy = (y0 - r + i) % N; if (yy < 0) yy += N;
+        int xx = (x0 - r + j) % N; if (xx < 0) xx += N;
+        tile[t] = F[(size_t)yy * N + xx];
+    }
+    __syncthreads();
+    const int lx = threadIdx.x;
+    for (int i = threadIdx.y; i < TH; i += CV_ROWS) {
+        float h = 0.f;
+        for (int kb = 0; kb < K; ++kb) h = fmaf(fac[kb], tile[i * TW + (lx + 2 * r - kb)], h);
+        hrow[i * CV_TX + lx] = h;
+    }
+    __syncthreads();
+    float acc[CV_TY / CV_ROWS];
+#pragma unroll
+    for (int q = 0; q < CV_TY / CV_ROWS; ++q) acc[q] = 0.f;
+    for (int ka = 0; ka < K; ++ka) {
+        const float w = fac[K + ka];
+#pragma unroll
+        for (int q = 0; q < CV_TY / CV_ROWS; ++q) {
+            const int ly = threadIdx.y + q * CV_ROWS;
+            acc[q] = fmaf(w, hrow[(ly + 2 * r - ka) * CV_TX + lx], acc[q]);
+        }
+    }
+    noise_mag_epilogue(a, acc, x0, y0, lx, m, b, mb);
+}
+
+// Stage 5 for the CV_TY / CV_ROWS outputs of one thread (R-Q11): sky, noise, magnitude.
+__device__ __forceinline__ void noise_mag_epilogue(const CvArgs &a, const float (&acc)[CV_TY / CV_ROWS], int x0, int y0,
+                                                   int lx, int m, int b, int mb) {
+    const int N = a.N;
     const int x = x0 + lx;
     if (x >= N) return;
     const uint32_t mctr = a.model0 + (uint32_t)m;
@@ -92,7 +145,7 @@ __global__ void __launch_bounds__(CV_TX * CV_ROWS) k_conv_noise(const CvArgs a) 
 int pcmd_launch_conv_noise(pcmd_ctx *c, int n_models, uint64_t seed, uint32_t model0, float *d_mag,
                            cudaStream_t s) {
     CvArgs a;
-    a.F = c->d_fdust; a.psf = c->d_psf; a.mag = d_mag; a.tap_conv = c->tap_conv;
+    a.F = c->d_fdust; a.psf = c->d_psf; a.psf_sep = c->d_psf_sep; a.mag = d_mag; a.tap_conv = c->tap_conv;
     a.sky_tab = c->d_sky_tab;
     for (int b = 0; b < 4; ++b) {
         a.sky_rec[b] = c->sky_rec[b];
@@ -102,14 +155,24 @@ int pcmd_launch_conv_noise(pcmd_ctx *c, int n_models, uint64_t seed, uint32_t mo
     a.shot_noise = c->shot_noise; a.poisson_sky = c->poisson_sky;
     a.key0 = (uint32_t)(seed & 0xFFFFFFFFull); a.key1 = (uint32_t)(seed >> 32); a.model0 = model0;
     const int K = c->K;
-    size_t smem = ((size_t)(CV_TX + K - 1) * (CV_TY + K - 1) + (size_t)K * K) * sizeof(float);
-    static size_t smem_set = 0;
-    if (smem > 48 * 1024 && smem > smem_set) {
-        PCMD_CUDA(c, cudaFuncSetAttribute(k_conv_noise, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        smem_set = smem;
-    }
     dim3 grid((c->N + CV_TX - 1) / CV_TX, (c->N + CV_TY - 1) / CV_TY, n_models * c->B);
-    k_conv_noise<<<grid, dim3(CV_TX, CV_ROWS), smem, s>>>(a);
+    if (c->psf_sep) {
+        size_t smem = ((size_t)(CV_TX + K - 1) * (CV_TY + K - 1) + (size_t)(CV_TY + K - 1) * CV_TX + 2 * (size_t)K) * sizeof(float);
+        static size_t smem_set_sep = 0;
+        if (smem > 48 * 1024 && smem > smem_set_sep) {
+            PCMD_CUDA(c, cudaFuncSetAttribute(k_conv_noise_sep, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+            smem_set_sep = smem;
+        }
+        k_conv_noise_sep<<<grid, dim3(CV_TX, CV_ROWS), smem, s>>>(a);
+    } else {
+        size_t smem = ((size_t)(CV_TX + K - 1) * (CV_TY + K - 1) + (size_t)K * K) * sizeof(float);
+        static size_t smem_set = 0;
+        if (smem > 48 * 1024 && smem > smem_set) {
+            PCMD_CUDA(c, cudaFuncSetAttribute(k_conv_noise, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+            smem_set = smem;
+        }
+        k_conv_noise<<<grid, dim3(CV_TX, CV_ROWS), smem, s>>>(a);
+    }
     PCMD_LAUNCHED(c);
     return PCMD_OK;
 }

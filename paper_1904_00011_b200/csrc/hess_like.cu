@@ -72,16 +72,25 @@ __global__ void __launch_bounds__(HS_THREADS) k_hess(const float *__restrict__ m
 
 __global__ void k_hess_stats(const pcmd_hess_stats *__restrict__ part, int nblk,
                              pcmd_hess_stats *__restrict__ out) {
-    // one thread per (model, hess): partials added in block order
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= (int)gridDim.y) { /* unused */ }
-    pcmd_hess_stats st = {0, 0, 0, 0, 0.0, 0.0};
+    // one warp per (model, hess): lane l adds partials l, l+32, ... in order, then a shuffle tree
+    // (a fixed order: deterministic sums)
     const pcmd_hess_stats *p = part + (size_t)blockIdx.x * nblk;
+    uint32_t n_in = 0, n_out = 0, n_bad = 0;
+    double sx = 0.0, sy = 0.0;
+    for (int b = threadIdx.x; b < nblk; b += 32) {
+        n_in += p[b].n_in; n_out += p[b].n_out; n_bad += p[b].n_bad;
+        sx += p[b].sum_x; sy += p[b].sum_y;
+    }
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) {
+        n_in += __shfl_down_sync(0xffffffffu, n_in, d);
+        n_out += __shfl_down_sync(0xffffffffu, n_out, d);
+        n_bad += __shfl_down_sync(0xffffffffu, n_bad, d);
+        sx += __shfl_down_sync(0xffffffffu, sx, d);
+        sy += __shfl_down_sync(0xffffffffu, sy, d);
+    }
     if (threadIdx.x == 0) {
-        for (int b = 0; b < nblk; ++b) {
-            st.n_in += p[b].n_in; st.n_out += p[b].n_out; st.n_bad += p[b].n_bad;
-            st.sum_x += p[b].sum_x; st.sum_y += p[b].sum_y;
-        }
+        pcmd_hess_stats st = {n_in, n_out, n_bad, 0, sx, sy};
         out[blockIdx.x] = st;
     }
 }
@@ -123,7 +132,7 @@ int pcmd_launch_hess(pcmd_ctx *c, const float *d_mag, int n_models, uint32_t *d_
 
 // ---------------------------------------------------------------------------------------------
 // Stage 7.  One block per model; every reduction is a fixed-order tree (deterministic).
-#define LL_THREADS 256
+#define LL_THREADS 1024
 
 __device__ double block_sum(double v, double *scratch) {
 #pragma unroll

@@ -60,7 +60,8 @@ struct pcmd_ctx {
     // ---- device constants
     int32_t *d_age_idx, *d_feh_idx;
     double *d_imf_w, *d_absmag, *d_feh_grid;
-    float *d_psf;          // [B][K][K] or [B][2][K]
+    float *d_psf;          // [B][K][K] (a separable PSF expanded)
+    float *d_psf_sep;      // [B][2][K] row and column factors of a separable PSF, else NULL
     uint64_t *d_mult;      // [Jpad] splitmix64(j)|1
     DevHess *d_hess_spec;  // [n_hess]
     uint32_t *d_sky_tab;   // [B][sky_cap] stored thresholds minus 1 of Poisson(sky_b)
