@@ -175,6 +175,22 @@ def shard_models(batch: int, rank: int) -> int:
     return rank * batch
 
 
+def max_over_ranks(x: float, device=None) -> float:
+    """Timing of a multi-rank job = the slowest rank (all_reduce MAX); identity for one rank."""
+    import torch
+    import torch.distributed as dist
+    if not (dist.is_available() and dist.is_initialized()) or dist.get_world_size() == 1:
+        return float(x)
+    t = torch.tensor([x], dtype=torch.float64, device=device or "cpu")
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_rate(units_per_rank: float, world: int, seconds: float) -> float:
+    """Whole-job throughput: units of ALL ranks over the slowest rank's time."""
+    return units_per_rank * world / seconds
+
+
 def batch_params(wl: dict, batch: int):
     prm = wl["params"]
     return [prm[i % len(prm)] for i in range(batch)]
@@ -248,11 +264,7 @@ def run_ours(args):
     launches = g.launch_count() - l0
     clk = clocks.stop(t_wall0, t_wall1)
     ms = np.array([a.elapsed_time(b) for a, b in ev])
-    total_ms = float(ms.sum())
-    if world > 1:
-        t = torch.tensor([total_ms], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms = float(t.item())
+    total_ms = max_over_ranks(float(ms.sum()), "cuda")
     g.profile(False)
 
     # ---- end to end through the host-buffer entry point
@@ -263,18 +275,14 @@ def run_ours(args):
     for _ in range(args.steps):
         lnl_h, H_h, st_h = g.evaluate_host(prm, data, seed=seed, model_index0=m0)
     torch.cuda.synchronize()
-    e2e_s = time.perf_counter() - t0
-    if world > 1:
-        t = torch.tensor([e2e_s], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_s = float(t.item())
+    e2e_s = max_over_ranks(time.perf_counter() - t0, "cuda")
     h2d = data.nbytes + n * (g.A * 8 + 5 * 8)
     d2h = n * (8 + g.bins_total * 4 + len(g.hess_specs) * 32)
 
     if rank == 0:
         peaks, which = measured_peaks()
         ms_step = total_ms / args.steps
-        evals = n * world * args.steps / (total_ms * 1e-3)
+        evals = whole_job_rate(n * args.steps, world, total_ms * 1e-3)
         s2_ms = float(stage[1]) / args.steps
         draws = draws_step
         ia = i_alg(g.B)
