@@ -323,6 +323,43 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
+def run_hbm_stages(args):
+    """HBM fraction of stages 4-5 and 6 on an L2-exceeding batch: the images of
+    `--hbm-batch` models of config `--config` geometry (default c4: 256x256 px, 2 bands) exceed the L2
+    several times, so every stage streams from / to HBM.  Prints one JSON line."""
+    import torch
+    import paper_1904_00011_b200 as G
+    torch.cuda.set_device(0)
+    wl = W.config(args.config)
+    g = G.Pcmd(wl, separable=True)
+    n = args.hbm_batch
+    prm = batch_params(wl, n)
+    mag = torch.empty((n, g.B, g.N, g.N), dtype=torch.float32, device="cuda")
+    H = torch.empty((n, g.bins_total), dtype=torch.int32, device="cuda")
+    g.profile(True)
+    acc = np.zeros(5)
+    reps = max(args.steps, 3)
+    for it in range(2 + reps):
+        g.simulate(prm, seed=1, mag=mag)
+        g.hess(mag, out=H)
+        ms = g.stage_ms()
+        if it >= 2:
+            acc += np.maximum(ms, 0.0)
+    acc /= reps
+    peaks, which = measured_peaks()
+    img_bytes = n * g.B * g.P * 4
+    used = len({b for h in g.hess_specs for b in (h["band_plus"], h["band_minus"], h["band_y"])})
+    s45 = 2 * img_bytes / (acc[2] * 1e-3) / 1e9
+    s6 = (n * len(g.hess_specs) * 0 + n * used * g.P * 4 + n * g.bins_total * 4) / (acc[3] * 1e-3) / 1e9
+    print(json.dumps({"hbm_stages": {
+        "workload": "c%d geometry x %d models (%.0f MB of images, L2 126 MB)" % (args.config, n, img_bytes / 1e6),
+        "stage4_5": {"ms": float(acc[2]), "algorithmic_bytes": 2 * img_bytes, "GBps": s45, "frac": s45 / peaks["hbm_gbs"]},
+        "stage6": {"ms": float(acc[3]), "algorithmic_bytes": n * used * g.P * 4 + n * g.bins_total * 4, "GBps": s6,
+                   "frac": s6 / peaks["hbm_gbs"]},
+        "stage2_ms": float(acc[1]), "peak_GBps": peaks["hbm_gbs"], "peak_source": which}}), flush=True)
+    g.close()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -334,8 +371,12 @@ def main():
     ap.add_argument("--cpu-sample", type=int, default=256, help="image side of the cpu_baseline sample")
     ap.add_argument("--ref-sample", type=int, default=128, help="image side of the --impl reference sample")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--hbm-batch", type=int, default=0,
+                    help="instead of the benchmark: HBM fraction of stages 4-6 on this many models (L2-exceeding)")
     args = ap.parse_args()
-    if args.impl == "reference":
+    if args.hbm_batch > 0:
+        run_hbm_stages(args)
+    elif args.impl == "reference":
         run_reference(args)
     else:
         run_ours(args)

@@ -7,6 +7,15 @@
 #define CV_TY 32
 #define CV_ROWS 8   // blockDim.y; each thread computes CV_TY / CV_ROWS outputs
 
+// v mod N for v in [-N, 2N) by one conditional add/subtract; the general case (image smaller than
+// the PSF halo) falls back to the division.
+__device__ __forceinline__ int wrap_index(int v, int N) {
+    if (v < 0) v += N;
+    if (v >= N) v -= N;
+    if ((unsigned)v >= (unsigned)N) { v %= N; if (v < 0) v += N; }
+    return v;
+}
+
 struct CvArgs {
     const float *F;      // [n_models][B][P] dusty flux
     const float *psf;    // [B][K][K]
@@ -36,11 +45,9 @@ __global__ void __launch_bounds__(CV_TX * CV_ROWS) k_conv_noise(const CvArgs a) 
     const int x0 = blockIdx.x * CV_TX, y0 = blockIdx.y * CV_TY;
     const int tid = threadIdx.y * CV_TX + threadIdx.x, nt = CV_TX * CV_ROWS;
     for (int t = tid; t < K * K; t += nt) spsf[t] = a.psf[(size_t)b * K * K + t];
-    for (int t = tid; t < TH * TW; t += nt) {
-        int i = t / TW, j = t - i * TW;
-        int yy = (y0 - r + i) % N; if (yy < 0) yy += N;
-        int xx = (x0 - r + j) % N; if (xx < 0) xx += N;
-        tile[t] = F[(size_t)yy * N + xx];
+    for (int i = threadIdx.y; i < TH; i += CV_ROWS) {      // halo tile with circular wrap (R-Q9)
+        const float *row = F + (size_t)wrap_index(y0 - r + i, N) * N;
+        for (int j = threadIdx.x; j < TW; j += CV_TX) tile[i * TW + j] = row[wrap_index(x0 - r + j, N)];
     }
     __syncthreads();
     const int lx = threadIdx.x;
@@ -61,9 +68,10 @@ __global__ void __launch_bounds__(CV_TX * CV_ROWS) k_conv_noise(const CvArgs a) 
 
 // Separable PSF (column factor (x) row factor, R-Q10): row pass over the halo tile into shared
 // memory, then the column pass: 2K FMAs per output instead of K^2.  Same tile, halo and epilogue.
+template <int KT>
 __global__ void __launch_bounds__(CV_TX * CV_ROWS) k_conv_noise_sep(const CvArgs a) {
     extern __shared__ float sm[];
-    const int K = a.K, r = (K - 1) / 2, N = a.N;
+    const int K = KT ? KT : a.K, r = (K - 1) / 2, N = a.N;
     const int TW = CV_TX + K - 1, TH = CV_TY + K - 1;
     float *tile = sm;                  // [TH][TW]
     float *hrow = sm + TH * TW;        // [TH][CV_TX] row-convolved
@@ -73,16 +81,15 @@ __global__ void __launch_bounds__(CV_TX * CV_ROWS) k_conv_noise_sep(const CvArgs
     const int x0 = blockIdx.x * CV_TX, y0 = blockIdx.y * CV_TY;
     const int tid = threadIdx.y * CV_TX + threadIdx.x, nt = CV_TX * CV_ROWS;
     for (int t = tid; t < 2 * K; t += nt) fac[t] = a.psf_sep[(size_t)b * 2 * K + t];
-    for (int t = tid; t < TH * TW; t += nt) {
-        int i = t / TW, j = t - i * TW;
-        int yy = (y0 - r + i) % N; if (yy < 0) yy += N;
-        int xx = (x0 - r + j) % N; if (xx < 0) xx += N;
-        tile[t] = F[(size_t)yy * N + xx];
+    for (int i = threadIdx.y; i < TH; i += CV_ROWS) {      // halo tile with circular wrap (R-Q9)
+        const float *row = F + (size_t)wrap_index(y0 - r + i, N) * N;
+        for (int j = threadIdx.x; j < TW; j += CV_TX) tile[i * TW + j] = row[wrap_index(x0 - r + j, N)];
     }
     __syncthreads();
     const int lx = threadIdx.x;
     for (int i = threadIdx.y; i < TH; i += CV_ROWS) {
         float h = 0.f;
+#pragma unroll
         for (int kb = 0; kb < K; ++kb) h = fmaf(fac[kb], tile[i * TW + (lx + 2 * r - kb)], h);
         hrow[i * CV_TX + lx] = h;
     }
@@ -90,6 +97,7 @@ __global__ void __launch_bounds__(CV_TX * CV_ROWS) k_conv_noise_sep(const CvArgs
     float acc[CV_TY / CV_ROWS];
 #pragma unroll
     for (int q = 0; q < CV_TY / CV_ROWS; ++q) acc[q] = 0.f;
+#pragma unroll
     for (int ka = 0; ka < K; ++ka) {
         const float w = fac[K + ka];
 #pragma unroll
@@ -109,6 +117,7 @@ __device__ __forceinline__ void noise_mag_epilogue(const CvArgs &a, const float 
     if (x >= N) return;
     const uint32_t mctr = a.model0 + (uint32_t)m;
     const double sky = a.sky[b], rs = a.read_sigma[b], zp = a.zp[b];
+    const float skyf = (float)sky, rs2 = (float)(rs * rs);
     const bool psky = a.poisson_sky && sky > 0.0;
     const bool need_g = a.shot_noise || rs > 0.0;
 #pragma unroll
@@ -118,27 +127,27 @@ __device__ __forceinline__ void noise_mag_epilogue(const CvArgs &a, const float 
         const uint32_t p = (uint32_t)y * (uint32_t)N + (uint32_t)x;
         const size_t o = (size_t)mb * a.P + p;
         if (a.tap_conv) a.tap_conv[o] = acc[q];
-        const double Gi = (double)acc[q];
+        // fp32 arithmetic (the noise term is a few per cent of the counts, so a
+        // 1e-7 error of the normal moves the magnitude by < 1e-8); only zp - 2.5 log10 is finished in fp64
+        const float Gi = acc[q];
         uint32_t w[4];
-        double g = 0.0;
+        float g = 0.f;
         if (need_g) {
             philox4x32_10(a.key0, a.key1, p, (uint32_t)b, mctr, 2u, w);
-            g = normal_from_words(w[0], w[1]);
+            g = normal_f32(w[0], w[1]);
         }
-        double Cp;
+        float arg;      // C' - sky
         if (psky) {
             philox4x32_10(a.key0, a.key1, p, (uint32_t)b, mctr, 3u, w);
             const PointRec sr = a.sky_rec[b];
-            double Kc = (double)(sr.k0 + count_below(a.sky_tab + sr.off, sr.len, w[0]));
-            double var = (a.shot_noise ? fmax(Gi, 0.0) : 0.0) + rs * rs;
-            Cp = Gi + Kc + sqrt(var) * g;
+            const float Kc = (float)(sr.k0 + count_below(a.sky_tab + sr.off, sr.len, w[0]));
+            const float var = (a.shot_noise ? fmaxf(Gi, 0.f) : 0.f) + rs2;
+            arg = Gi + (Kc - skyf) + sqrtf(var) * g;
         } else {
-            double C = Gi + sky;
-            double var = (a.shot_noise ? fmax(C, 0.0) : 0.0) + rs * rs;
-            Cp = C + sqrt(var) * g;
+            const float var = (a.shot_noise ? fmaxf(Gi + skyf, 0.f) : 0.f) + rs2;
+            arg = Gi + sqrtf(var) * g;
         }
-        double arg = Cp - sky;
-        a.mag[o] = (arg > 0.0) ? (float)(zp - 2.5 * log10(arg)) : __int_as_float(0x7fc00000);
+        a.mag[o] = (arg > 0.f) ? (float)fma((double)log2_pos(arg), -0.75257498915995298, zp) : __int_as_float(0x7fc00000);
     }
 }
 
@@ -158,12 +167,19 @@ int pcmd_launch_conv_noise(pcmd_ctx *c, int n_models, uint64_t seed, uint32_t mo
     dim3 grid((c->N + CV_TX - 1) / CV_TX, (c->N + CV_TY - 1) / CV_TY, n_models * c->B);
     if (c->psf_sep) {
         size_t smem = ((size_t)(CV_TX + K - 1) * (CV_TY + K - 1) + (size_t)(CV_TY + K - 1) * CV_TX + 2 * (size_t)K) * sizeof(float);
-        static size_t smem_set_sep = 0;
-        if (smem > 48 * 1024 && smem > smem_set_sep) {
-            PCMD_CUDA(c, cudaFuncSetAttribute(k_conv_noise_sep, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-            smem_set_sep = smem;
+        const dim3 blk(CV_TX, CV_ROWS);
+        if (K == 5) k_conv_noise_sep<5><<<grid, blk, smem, s>>>(a);
+        else if (K == 7) k_conv_noise_sep<7><<<grid, blk, smem, s>>>(a);
+        else if (K == 15) k_conv_noise_sep<15><<<grid, blk, smem, s>>>(a);
+        else if (K == 21) k_conv_noise_sep<21><<<grid, blk, smem, s>>>(a);
+        else {
+            static size_t smem_set_sep = 0;
+            if (smem > 48 * 1024 && smem > smem_set_sep) {
+                PCMD_CUDA(c, cudaFuncSetAttribute(k_conv_noise_sep<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+                smem_set_sep = smem;
+            }
+            k_conv_noise_sep<0><<<grid, blk, smem, s>>>(a);
         }
-        k_conv_noise_sep<<<grid, dim3(CV_TX, CV_ROWS), smem, s>>>(a);
     } else {
         size_t smem = ((size_t)(CV_TX + K - 1) * (CV_TY + K - 1) + (size_t)K * K) * sizeof(float);
         static size_t smem_set = 0;

@@ -10,7 +10,7 @@
 // x = fl(mp - mm); t = fl(fl(x - x_lo) * inv_dx); ix = floor(t); half-open.
 template <bool SMEM>
 __global__ void __launch_bounds__(HS_THREADS) k_hess(const float *__restrict__ mag, int B, int64_t P,
-                                                     const DevHess *__restrict__ specs, int n_hess,
+                                                     const DevHess *__restrict__ specs, int n_hess, int64_t ppb,
                                                      int64_t bins_total, uint32_t *__restrict__ hess,
                                                      pcmd_hess_stats *__restrict__ part) {
     extern __shared__ uint32_t sh[];
@@ -27,18 +27,31 @@ __global__ void __launch_bounds__(HS_THREADS) k_hess(const float *__restrict__ m
     const float *my = mag + ((size_t)m * B + S.band_y) * P;
     uint32_t n_in = 0, n_out = 0, n_bad = 0;
     double sx = 0.0, sy = 0.0;
-    const int64_t p0 = (int64_t)blockIdx.x * HS_PIX_PER_BLOCK;
-    const int64_t p1 = min(P, p0 + HS_PIX_PER_BLOCK);
-    for (int64_t p = p0 + threadIdx.x; p < p1; p += HS_THREADS) {
-        const float a = mp[p], b = mm[p], y = my[p];
-        if (isnan(a) || isnan(b) || isnan(y)) { n_bad++; continue; }
+    const int64_t p0 = (int64_t)blockIdx.x * ppb;
+    const int64_t p1 = min(P, p0 + ppb);
+    auto one = [&](float a, float b, float y) {
+        if (isnan(a) || isnan(b) || isnan(y)) { n_bad++; return; }
         const float x = __fsub_rn(a, b);
         const float fx = floorf(__fmul_rn(__fsub_rn(x, S.x_lo), S.inv_dx));
         const float fy = floorf(__fmul_rn(__fsub_rn(y, S.y_lo), S.inv_dy));
-        if (!(fx >= 0.0f) || !(fx < (float)S.nx) || !(fy >= 0.0f) || !(fy < (float)S.ny)) { n_out++; continue; }
+        if (!(fx >= 0.0f) || !(fx < (float)S.nx) || !(fy >= 0.0f) || !(fy < (float)S.ny)) { n_out++; return; }
         const int bin = (int)fy * S.nx + (int)fx;
         if (SMEM) atomicAdd(&sh[bin], 1u); else atomicAdd(&gh[bin], 1u);
         n_in++; sx += (double)x; sy += (double)y;
+    };
+    if (((P | p0) & 3) == 0) {      // 16-byte loads: every row of every image starts 16-byte aligned
+        const float4 *vp = reinterpret_cast<const float4 *>(mp), *vm = reinterpret_cast<const float4 *>(mm),
+                     *vy = reinterpret_cast<const float4 *>(my);
+        const int64_t q1 = (p1 + 3) >> 2;
+        for (int64_t q = (p0 >> 2) + threadIdx.x; q < q1; q += HS_THREADS) {
+            const float4 A = vp[q], Bv = vm[q], Y = vy[q];
+            one(A.x, Bv.x, Y.x);
+            if (4 * q + 1 < p1) one(A.y, Bv.y, Y.y);
+            if (4 * q + 2 < p1) one(A.z, Bv.z, Y.z);
+            if (4 * q + 3 < p1) one(A.w, Bv.w, Y.w);
+        }
+    } else {
+        for (int64_t p = p0 + threadIdx.x; p < p1; p += HS_THREADS) one(mp[p], mm[p], my[p]);
     }
     // block reduction of the stats in a fixed order (deterministic)
     __shared__ double r_sx[HS_THREADS / 32], r_sy[HS_THREADS / 32];
@@ -97,7 +110,13 @@ __global__ void k_hess_stats(const pcmd_hess_stats *__restrict__ part, int nblk,
 
 int pcmd_launch_hess(pcmd_ctx *c, const float *d_mag, int n_models, uint32_t *d_hess,
                      pcmd_hess_stats *d_stats, cudaStream_t s) {
-    const int nblk = (int)((c->P + HS_PIX_PER_BLOCK - 1) / HS_PIX_PER_BLOCK);
+    // pixels per block: at least HS_PIX_PER_BLOCK, more when the batch alone fills the GPU (a block
+    // zeroes and flushes a whole private histogram, so long pixel runs amortise that)
+    int64_t want_blocks = ((int64_t)c->sm_count * 8 + (int64_t)n_models * c->n_hess - 1) / ((int64_t)n_models * c->n_hess);
+    int64_t ppb = (c->P + want_blocks - 1) / want_blocks;
+    if (ppb < HS_PIX_PER_BLOCK) ppb = HS_PIX_PER_BLOCK;
+    ppb = (ppb + 1023) & ~(int64_t)1023;
+    const int nblk = (int)((c->P + ppb - 1) / ppb);
     const int64_t need = (int64_t)n_models * c->n_hess * nblk;
     if (need > c->hpart_cap) {
         if (c->d_hpart) cudaFree(c->d_hpart);
@@ -116,10 +135,10 @@ int pcmd_launch_hess(pcmd_ctx *c, const float *d_mag, int n_models, uint32_t *d_
             PCMD_CUDA(c, cudaFuncSetAttribute(k_hess<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
             smem_set = smem;
         }
-        k_hess<true><<<grid, HS_THREADS, smem, s>>>(d_mag, c->B, c->P, c->d_hess_spec, c->n_hess,
+        k_hess<true><<<grid, HS_THREADS, smem, s>>>(d_mag, c->B, c->P, c->d_hess_spec, c->n_hess, ppb,
                                                     c->hess_bins, d_hess, c->d_hpart);
     } else {
-        k_hess<false><<<grid, HS_THREADS, 0, s>>>(d_mag, c->B, c->P, c->d_hess_spec, c->n_hess,
+        k_hess<false><<<grid, HS_THREADS, 0, s>>>(d_mag, c->B, c->P, c->d_hess_spec, c->n_hess, ppb,
                                                   c->hess_bins, d_hess, c->d_hpart);
     }
     PCMD_LAUNCHED(c);

@@ -158,6 +158,25 @@ __device__ __forceinline__ double normal_from_words(uint32_t w0, uint32_t w1) {
     return sqrt(-2.0 * log(u1)) * cos(6.283185307179586476925 * u2);
 }
 
+// The same normal in fp32 (stages 3 and 5).  Special-function-unit approximations: ln with an
+// absolute error of ~1e-7 on -ln u (relative 1e-6 near u = 1), cos with ~2e-6; the normal is good to
+// ~2e-6, which moves a magnitude by < 1e-7 when the noise is a few per cent of the counts
+// (DESIGN.md "Tolerances").
+__device__ __forceinline__ float normal_f32(uint32_t w0, uint32_t w1) {
+    const float u1 = fminf(((float)w0 + 0.5f) * 2.3283064365386963e-10f, 0.99999994f);
+    const float u2 = ((float)w1 + 0.5f) * 2.3283064365386963e-10f;
+    const float L = -1.3862943611198906f * __log2f(u1);          // -2 ln u1 = -2 ln2 log2 u1
+    return L * rsqrtf(L) * __cosf(6.2831853071795865f * u2 - 3.1415926535897932f) * -1.0f;   // cos(x) = -cos(x - pi)
+}
+
+// log2 of a positive normal float with an absolute error of ~2.4e-7: exponent exactly, mantissa by
+// the special-function unit (whose absolute error bound holds on [0.5, 2]).
+__device__ __forceinline__ float log2_pos(float x) {
+    const int e = (int)((__float_as_uint(x) >> 23) & 0xFFu) - 127;
+    const float mant = __uint_as_float((__float_as_uint(x) & 0x007FFFFFu) | 0x3F800000u);
+    return (float)e + __log2f(mant);
+}
+
 // #{i < len : u > T[i]} for non-decreasing T (thresholds stored minus 1)
 __device__ __forceinline__ uint32_t count_below(const uint32_t *__restrict__ T, uint32_t len, uint32_t u) {
     uint32_t lo = 0, hi = len;

@@ -347,14 +347,15 @@ __global__ void __launch_bounds__(256) k_reduce_dust(const RdArgs a) {
     const int m = (int)(idx / a.P);
     const uint32_t p = (uint32_t)(idx - (int64_t)m * a.P);
     const int n_seg = a.seg[m].n_seg;
-    double A = 0.0; bool behind = true;
-    if (a.dust_mode != 0) {
+    float A = 0.f; bool behind = true;
+    if (a.dust_mode != 0) {       // fp32: the factor needs 1e-5 relative, expf / exp10f give 1e-7
         const DevModel M = a.mdl[m];
         uint32_t w[4];
         philox4x32_10(a.key0, a.key1, p, 0u, a.model0 + (uint32_t)m, 1u, w);
-        A = M.dust_med * exp(M.dust_sigma * normal_from_words(w[0], w[1]));
+        A = (float)M.dust_med * expf((float)M.dust_sigma * normal_f32(w[0], w[1]));
         if (a.dust_mode == 2) behind = ((double)w[2] < a.dust_frac * 4294967296.0);
     }
+    const float Fd = (float)a.dust_frac;
     for (int b = 0; b < a.B; ++b) {
         double s = 0.0;
         for (int sg = 0; sg < n_seg; ++sg)
@@ -362,10 +363,10 @@ __global__ void __launch_bounds__(256) k_reduce_dust(const RdArgs a) {
         const float F = (float)s;
         const size_t o = ((size_t)m * a.B + b) * a.P + p;
         if (a.flux_raw) a.flux_raw[o] = F;
-        double fac = 1.0;
-        if (a.dust_mode == 1) fac = (1.0 - a.dust_frac) + a.dust_frac * pow(10.0, -0.4 * a.coef[b] * A);
-        else if (a.dust_mode == 2) fac = behind ? pow(10.0, -0.4 * a.coef[b] * A) : 1.0;
-        a.flux_dust[o] = (float)((double)F * fac);
+        float fac = 1.f;
+        if (a.dust_mode == 1) fac = (1.f - Fd) + Fd * exp10f(-0.4f * (float)a.coef[b] * A);
+        else if (a.dust_mode == 2) fac = behind ? exp10f(-0.4f * (float)a.coef[b] * A) : 1.f;
+        a.flux_dust[o] = F * fac;
     }
 }
 
