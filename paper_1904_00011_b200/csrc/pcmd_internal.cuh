@@ -18,17 +18,18 @@ struct __align__(16) PointRec {
 // Stage-2 work layout.  Groups of four consecutive isochrone points (one
 // Philox call, R-C1) are classified by how many sampler thresholds decide almost every draw and
 // sorted by class; a class is cut into segments; one (model, pixel tile, segment) is a work unit.
-#define S2_NCLASS 7        // classes, most expensive first:
+#define S2_NCLASS 8        // classes, most expensive first:
 #define S2_CLS_D9 1        //   0 bisection in global memory (tables longer than 511)
 #define S2_CLS_D7 2        //   1-3 branch-free search of a padded table of 2^D words in shared memory
 #define S2_CLS_D5 3
 #define S2_CLS_L4 4        //   4-6 L inline thresholds decide the draw (more stars: probability < 2^-10)
 #define S2_CLS_L2 5
 #define S2_CLS_L1 6
-#define S2_CLS_NONE 7      //   no point of the group can have a star: dropped
+#define S2_CLS_L0 7        //   7 rare: P(any star) < 2^-8 per draw: one max-compare per group, then class L1's path
+#define S2_CLS_NONE 8      //   no point of the group can have a star: dropped
 #define S2_SEG_MAX 48      // segments per model (all classes together)
 struct __align__(16) GroupRec {      // 160 bytes
-    uint32_t g_orig, cls, pad0, pad1; // original group index (Philox counter word 1), class
+    uint32_t g_orig, cls, tmin, pad1; // original group index (Philox counter word 1), class, min over w of T[0][w]
     uint32_t T[5][4];                 // T[i][w]: (i+1)-th stored threshold minus 1 of point w; 0xFFFFFFFF if none
     float f[4][4];                    // f[w][b]: flux of one star of point w in band b
 };

@@ -210,9 +210,15 @@ __global__ void k_table_compact(int J, int n_models, const uint32_t *__restrict_
 #endif
 #define S2_OVF_THR (0xFFFFFFFFu - (1u << (32 - S2_OVF_LOG2)))   /* 2^32 (1 - 2^-10) - 1 */
 
+#ifndef S2_RARE_LOG2
+#define S2_RARE_LOG2 8
+#endif
+#define S2_RARE_THR (0xFFFFFFFFu - (1u << (32 - S2_RARE_LOG2)))   /* P(any star) < 2^-8 per draw */
+
 __device__ __forceinline__ int point_class(const PointRec &r, const uint32_t *__restrict__ tab) {
     if (r.len == 0 && r.k0 == 0) return S2_CLS_NONE;      // never a star
     if (r.k0 == 0) {
+        if (r.T0 >= S2_RARE_THR && (r.len <= 1 || tab[r.off + 1] >= S2_OVF_THR)) return S2_CLS_L0;
         if (r.len <= 1 || tab[r.off + 1] >= S2_OVF_THR) return S2_CLS_L1;
         if (r.len <= 2 || tab[r.off + 2] >= S2_OVF_THR) return S2_CLS_L2;
         if (r.len <= 4 || tab[r.off + 4] >= S2_OVF_THR) return S2_CLS_L4;
@@ -301,7 +307,7 @@ __global__ void __launch_bounds__(1024) k_group_sort(const uint8_t *__restrict__
         t.cls_start[S2_NCLASS] = (int32_t)cls_start[S2_NCLASS];
         t.first_d = first_d;
         // segments: each class gets a share of seg_budget proportional to its estimated cost
-        const float wgt[S2_NCLASS] = {8.0f, 3.2f, 2.6f, 2.0f, 1.5f, 1.15f, 1.0f};
+        const float wgt[S2_NCLASS] = {8.0f, 3.2f, 2.6f, 2.0f, 1.5f, 1.15f, 1.0f, 0.8f};
         float total = 0.f;
         for (int c = 0; c < S2_NCLASS; ++c) {
             const float wc = (c >= 1 && c < first_d) ? wgt[0] : wgt[c];
@@ -347,7 +353,10 @@ __global__ void __launch_bounds__(256) k_group_emit(const PointRec *__restrict__
     if (lane < 4) {
         const int w = lane;
         const PointRec r = rec[4 * g + w];
-        if (w == 0) { o->g_orig = (uint32_t)g; o->cls = (uint32_t)cls; o->pad0 = o->pad1 = 0; }
+        uint32_t tmin = r.T0;                       // smallest first threshold of the four points
+        tmin = min(tmin, __shfl_xor_sync(0xFu, tmin, 1));
+        tmin = min(tmin, __shfl_xor_sync(0xFu, tmin, 2));
+        if (w == 0) { o->g_orig = (uint32_t)g; o->cls = (uint32_t)cls; o->tmin = tmin; o->pad1 = 0; }
 #pragma unroll
         for (int i = 0; i < 5; ++i) o->T[i][w] = ((uint32_t)i < r.len) ? tab[r.off + i] : 0xFFFFFFFFu;
         if (cls <= S2_CLS_D5) o->T[4][w] = r.k0;     // the search classes keep k0 here

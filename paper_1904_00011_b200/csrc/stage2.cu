@@ -165,6 +165,20 @@ __device__ __forceinline__ void group_short(S2State<NB, COUNTS> &st, const Group
     if (__any_sync(0xffffffffu, ovf)) overflow_fixup<NB, COUNTS, L>(st, g, u, rec, tab, mult);
 }
 
+// Class L0: a star anywhere in the group is rare (< 2^-8 per draw): one compare of the largest of
+// the thread's draws against the smallest first threshold, a vote, and class L1's path if any lane hit.
+template <int NB, bool COUNTS>
+__device__ __forceinline__ void group_rare(S2State<NB, COUNTS> &st, const GroupRec *__restrict__ g,
+                                           const uint32_t (&u)[S2_PX][4], const PointRec *__restrict__ rec,
+                                           const uint32_t *__restrict__ tab, const uint64_t *__restrict__ mult) {
+    uint32_t mx = 0;
+#pragma unroll
+    for (int i = 0; i < S2_PX; ++i)
+#pragma unroll
+        for (int w = 0; w < 4; ++w) mx = max(mx, u[i][w]);
+    if (__any_sync(0xffffffffu, mx > g->tmin)) group_short<NB, COUNTS, 1>(st, g, u, rec, tab, mult);
+}
+
 // Class L = 4: count the exceeded thresholds, one FMA per band.
 template <int NB, bool COUNTS>
 __device__ __forceinline__ void group_four(S2State<NB, COUNTS> &st, const GroupRec *__restrict__ g,
@@ -304,7 +318,8 @@ __global__ void __launch_bounds__(S2_THREADS, S2_MINB) k_stage2(const S2Args a) 
                 BODY;                                                                          \
                 if ((g & (S2_FLUSH - 1)) == S2_FLUSH - 1) st.flush();                          \
             }
-            if (cls == S2_CLS_L1) { S2_LOOP((group_short<NB, COUNTS, 1>(st, gr, u, rec, tab, a.mult))) }
+            if (cls == S2_CLS_L0) { S2_LOOP((group_rare<NB, COUNTS>(st, gr, u, rec, tab, a.mult))) }
+            else if (cls == S2_CLS_L1) { S2_LOOP((group_short<NB, COUNTS, 1>(st, gr, u, rec, tab, a.mult))) }
             else if (cls == S2_CLS_L2) { S2_LOOP((group_short<NB, COUNTS, 2>(st, gr, u, rec, tab, a.mult))) }
             else if (cls == S2_CLS_L4) { S2_LOOP((group_four<NB, COUNTS>(st, gr, u, rec, tab, a.mult))) }
             else if (cls == S2_CLS_D5) { S2_LOOP((group_search<NB, COUNTS, 5>(st, gr, u, xt, (uint32_t)g << 9, a.mult))) }
