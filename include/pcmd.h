@@ -107,6 +107,15 @@ int  pcmd_simulate(pcmd_ctx *ctx, const pcmd_params *params, int32_t n_models,
                    float *d_mag, float *d_flux_raw,
                    uint64_t *d_count_hash, uint32_t *d_count_total, void *cuda_stream);
 
+/* Repeated realisations of ONE parameter vector (Appendix A: "we recompute the
+ * likelihood of the best fit model 100 times"; the likelihood is stochastic):
+ * identical to pcmd_simulate with n_repeats copies of params[0] -- realisation r uses counter word
+ * model_index0 + r -- but stage 1 runs once.  Outputs are [n_repeats][...] like pcmd_simulate's. */
+int  pcmd_simulate_repeat(pcmd_ctx *ctx, const pcmd_params *params, int32_t n_repeats,
+                          uint64_t seed, uint32_t model_index0,
+                          float *d_mag, float *d_flux_raw,
+                          uint64_t *d_count_hash, uint32_t *d_count_total, void *cuda_stream);
+
 /* Stage 6: Hess diagrams of d_mag.
  *   d_hess   DEVICE out [n_models][hess_bins_total] uint32, the n_hess diagrams of a model one
  *            after another, each [ny][nx]; overwritten

@@ -76,6 +76,7 @@ def lib():
         L.pcmd_destroy.argtypes = [vp]
         L.pcmd_destroy.restype = None
         L.pcmd_simulate.argtypes = [vp, vp, i32, u64, u32, vp, vp, vp, vp, vp]
+        L.pcmd_simulate_repeat.argtypes = [vp, vp, i32, u64, u32, vp, vp, vp, vp, vp]
         L.pcmd_hess.argtypes = [vp, vp, i32, vp, vp, vp]
         L.pcmd_loglike.argtypes = [vp, vp, vp, i32, vp, vp, i32, vp, vp]
         L.pcmd_evaluate_host.argtypes = [vp, vp, i32, u64, u32, vp, vp, i32, vp, vp, vp, vp]
@@ -205,6 +206,22 @@ class Pcmd:
             out["flux_raw"] = raw
         if want_counts:
             out["hash"], out["total"] = hsh, tot
+        return out
+
+    def simulate_repeat(self, prm, n_repeats, seed=0, model_index0=0, want_raw=False, mag=None):
+        """n_repeats realisations of one parameter vector (stage 1 once)."""
+        t = self.torch
+        arr, keep = self._params([prm])
+        if mag is None:
+            mag = t.empty((n_repeats, self.B, self.N, self.N), dtype=t.float32, device="cuda")
+        raw = t.empty_like(mag) if want_raw else None
+        rc = lib().pcmd_simulate_repeat(self._ctx, C.addressof(arr), n_repeats, C.c_uint64(seed), model_index0,
+                                        _dp(mag), _dp(raw), None, None, self._stream())
+        if rc:
+            raise PcmdError(rc, "pcmd_simulate_repeat")
+        out = dict(mag=mag)
+        if want_raw:
+            out["flux_raw"] = raw
         return out
 
     def hess(self, mag, want_stats=True, out=None):

@@ -35,13 +35,13 @@ extern "C" const char *pcmd_strerror(int code) {
 static void free_scratch(pcmd_ctx *c) {
     cudaFree(c->d_sfh); cudaFree(c->d_model); cudaFree(c->d_mdfw); cudaFree(c->d_lambda);
     cudaFree(c->d_rawcnt); cudaFree(c->d_klo); cudaFree(c->d_q); cudaFree(c->d_stcnt);
-    cudaFree(c->d_tab); cudaFree(c->d_rec); cudaFree(c->d_fdust); cudaFree(c->d_grp); cudaFree(c->d_seg);
+    cudaFree(c->d_tab); cudaFree(c->d_rec); cudaFree(c->d_grp); cudaFree(c->d_seg);
     cudaFree(c->d_gcls); cudaFree(c->d_arena); cudaFree(c->d_gpos);
     c->d_grp = nullptr; c->d_seg = nullptr; c->d_gcls = nullptr; c->d_arena = nullptr; c->d_gpos = nullptr;
     if (c->h_stage) cudaFreeHost(c->h_stage);
     c->d_sfh = nullptr; c->d_model = nullptr; c->d_mdfw = nullptr; c->d_lambda = nullptr;
     c->d_rawcnt = nullptr; c->d_klo = nullptr; c->d_q = nullptr; c->d_stcnt = nullptr;
-    c->d_tab = nullptr; c->d_rec = nullptr; c->d_fdust = nullptr; c->h_stage = nullptr;
+    c->d_tab = nullptr; c->d_rec = nullptr; c->h_stage = nullptr;
     c->cap_models = 0; c->cap_raw = 0;
 }
 
@@ -63,7 +63,6 @@ static int ensure_scratch(pcmd_ctx *c, int n_models, int64_t cap_raw) {
     PCMD_CUDA(c, cudaMalloc(&c->d_q, (size_t)nm * cr * sizeof(double)));
     PCMD_CUDA(c, cudaMalloc(&c->d_tab, (size_t)nm * cr * sizeof(uint32_t)));
     PCMD_CUDA(c, cudaMalloc(&c->d_rec, (size_t)nm * Jp * sizeof(PointRec)));
-    PCMD_CUDA(c, cudaMalloc(&c->d_fdust, (size_t)nm * c->B * c->P * sizeof(float)));
     PCMD_CUDA(c, cudaMalloc(&c->d_grp, (size_t)nm * (Jp / 4) * sizeof(GroupRec)));
     PCMD_CUDA(c, cudaMalloc(&c->d_seg, (size_t)nm * sizeof(SegTable)));
     PCMD_CUDA(c, cudaMalloc(&c->d_gcls, (size_t)nm * (Jp / 4)));
@@ -194,7 +193,7 @@ extern "C" void pcmd_destroy(pcmd_ctx *c) {
     free_scratch(c);
     cudaFree(c->d_age_idx); cudaFree(c->d_feh_idx); cudaFree(c->d_imf_w); cudaFree(c->d_absmag);
     cudaFree(c->d_feh_grid); cudaFree(c->d_psf); cudaFree(c->d_psf_sep); cudaFree(c->d_mult); cudaFree(c->d_hess_spec);
-    cudaFree(c->d_sky_tab); cudaFree(c->d_status); cudaFree(c->d_hpart); cudaFree(c->d_part);
+    cudaFree(c->d_sky_tab); cudaFree(c->d_status); cudaFree(c->d_hpart); cudaFree(c->d_part); cudaFree(c->d_fdust);
     cudaFree(c->d_mag); cudaFree(c->d_hessbuf); cudaFree(c->d_statbuf); cudaFree(c->d_lnl);
     cudaFree(c->d_hess_data); cudaFree(c->d_data_stats);
     if (c->h_pin) cudaFreeHost(c->h_pin);
@@ -207,7 +206,9 @@ extern "C" void pcmd_destroy(pcmd_ctx *c) {
 // ---------------------------------------------------------------------------------------------
 
 
-static int stage_params(pcmd_ctx *c, const pcmd_params *params, int n_models, cudaStream_t s) {
+// n_models parameter vectors (tables), n_real realisations (images): n_real = n_models, or
+// n_models = 1 and n_real repeats of it (pcmd_simulate_repeat).
+static int stage_params(pcmd_ctx *c, const pcmd_params *params, int n_models, int n_real, cudaStream_t s) {
     // upper bound of the raw sampler-table size of one model (sizing only, no method arithmetic):
     // lambda_j <= max_a sfh_a * imf_w_j, and a table spans fewer than 20 sqrt(lambda) + 96 counts.
     int64_t cap = 0;
@@ -235,9 +236,16 @@ static int stage_params(pcmd_ctx *c, const pcmd_params *params, int n_models, cu
     if (cap > 0xFFFFFFF0ll) return PCMD_ERANGE;
     int rc = ensure_scratch(c, n_models, cap);
     if (rc) return rc;
-    c->seg_budget = pcmd_stage2_seg_budget(c, n_models);
+    c->seg_budget = pcmd_stage2_seg_budget(c, n_real);
     c->seg_cap = c->seg_budget + S2_NCLASS;
-    const int64_t need = (int64_t)n_models * c->seg_cap * c->B * c->P;
+    const int64_t need_img = (int64_t)n_real * c->B * c->P;
+    if (need_img > c->fdust_elems) {
+        cudaDeviceSynchronize();
+        cudaFree(c->d_fdust); c->d_fdust = nullptr; c->fdust_elems = 0;
+        PCMD_CUDA(c, cudaMalloc(&c->d_fdust, (size_t)need_img * sizeof(float)));
+        c->fdust_elems = need_img;
+    }
+    const int64_t need = (int64_t)n_real * c->seg_cap * c->B * c->P;
     if (need > c->part_elems) {
         cudaDeviceSynchronize();
         cudaFree(c->d_part); c->d_part = nullptr; c->part_elems = 0;
@@ -256,15 +264,15 @@ static int stage_params(pcmd_ctx *c, const pcmd_params *params, int n_models, cu
     return PCMD_OK;
 }
 
-extern "C" int pcmd_simulate(pcmd_ctx *c, const pcmd_params *params, int32_t n_models, uint64_t seed,
-                             uint32_t model_index0, float *d_mag, float *d_flux_raw,
-                             uint64_t *d_count_hash, uint32_t *d_count_total, void *cuda_stream) {
-    if (!c || !params || n_models < 1 || !d_mag) return PCMD_EINVAL;
+static int simulate_impl(pcmd_ctx *c, const pcmd_params *params, int32_t n_models, int32_t n_real, uint64_t seed,
+                         uint32_t model_index0, float *d_mag, float *d_flux_raw, uint64_t *d_count_hash,
+                         uint32_t *d_count_total, void *cuda_stream) {
+    if (!c || !params || n_models < 1 || n_real < 1 || !d_mag) return PCMD_EINVAL;
     if ((d_count_hash == nullptr) != (d_count_total == nullptr)) return PCMD_EINVAL;
     cudaStream_t s = (cudaStream_t)cuda_stream;
     // the pinned staging buffer is reused: wait until the previous call's copies have run
     if (c->stage_ev_valid) PCMD_CUDA(c, cudaEventSynchronize(c->stage_ev));
-    int rc = stage_params(c, params, n_models, s);
+    int rc = stage_params(c, params, n_models, n_real, s);
     if (rc) return rc;
     if (!c->stage_ev_valid) {
         PCMD_CUDA(c, cudaEventCreateWithFlags(&c->stage_ev, cudaEventDisableTiming));
@@ -273,17 +281,32 @@ extern "C" int pcmd_simulate(pcmd_ctx *c, const pcmd_params *params, int32_t n_m
     PCMD_CUDA(c, cudaEventRecord(c->stage_ev, s));
     PCMD_CUDA(c, cudaMemsetAsync(c->d_status, 0, 2 * sizeof(int32_t), s));
     c->last_models = n_models;
+    c->tab_stride = (n_models == n_real) ? 1 : 0;     // 0: every realisation reads model 0's tables
     PCMD_PROF(c, 0, s);
     if ((rc = pcmd_launch_stage1(c, n_models, s))) return rc;
     PCMD_PROF(c, 1, s);
-    if ((rc = pcmd_launch_stage2(c, n_models, seed, model_index0, d_flux_raw, d_count_hash, d_count_total, s))) return rc;
+    if ((rc = pcmd_launch_stage2(c, n_real, seed, model_index0, d_flux_raw, d_count_hash, d_count_total, s))) return rc;
     PCMD_PROF(c, 2, s);
     if (c->tap_dust)
-        PCMD_CUDA(c, cudaMemcpyAsync(c->tap_dust, c->d_fdust, (size_t)n_models * c->B * c->P * sizeof(float),
+        PCMD_CUDA(c, cudaMemcpyAsync(c->tap_dust, c->d_fdust, (size_t)n_real * c->B * c->P * sizeof(float),
                                      cudaMemcpyDeviceToDevice, s));
-    if ((rc = pcmd_launch_conv_noise(c, n_models, seed, model_index0, d_mag, s))) return rc;
+    if ((rc = pcmd_launch_conv_noise(c, n_real, seed, model_index0, d_mag, s))) return rc;
     PCMD_PROF(c, 3, s);
     return PCMD_OK;
+}
+
+extern "C" int pcmd_simulate(pcmd_ctx *c, const pcmd_params *params, int32_t n_models, uint64_t seed,
+                             uint32_t model_index0, float *d_mag, float *d_flux_raw,
+                             uint64_t *d_count_hash, uint32_t *d_count_total, void *cuda_stream) {
+    return simulate_impl(c, params, n_models, n_models, seed, model_index0, d_mag, d_flux_raw, d_count_hash,
+                         d_count_total, cuda_stream);
+}
+
+extern "C" int pcmd_simulate_repeat(pcmd_ctx *c, const pcmd_params *params, int32_t n_repeats, uint64_t seed,
+                                    uint32_t model_index0, float *d_mag, float *d_flux_raw,
+                                    uint64_t *d_count_hash, uint32_t *d_count_total, void *cuda_stream) {
+    return simulate_impl(c, params, 1, n_repeats, seed, model_index0, d_mag, d_flux_raw, d_count_hash,
+                         d_count_total, cuda_stream);
 }
 
 extern "C" int pcmd_hess(pcmd_ctx *c, const float *d_mag, int32_t n_models, uint32_t *d_hess,

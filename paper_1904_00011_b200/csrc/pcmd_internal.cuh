@@ -82,7 +82,8 @@ struct pcmd_ctx {
     uint32_t *d_stcnt;     // [cap_models][J+1] stored counts -> exclusive offsets
     uint32_t *d_tab;       // [cap_models][cap_raw] stored thresholds minus 1
     PointRec *d_rec;       // [cap_models][Jpad]
-    float *d_fdust;        // [cap_models][B][P]
+    float *d_fdust; int64_t fdust_elems;   // [realisations][B][P] dusty flux
+    int32_t tab_stride;    // 1: realisation m reads model m's tables; 0: all read model 0's (repeat mode)
     GroupRec *d_grp;       // [cap_models][Jpad/4] class-sorted group records
     SegTable *d_seg;       // [cap_models]
     uint8_t *d_gcls;       // [cap_models][Jpad/4] class of each group (original order)

@@ -34,7 +34,7 @@ struct S2Args {
     const uint64_t *mult;    // [Jpad]
     const uint32_t *arena;   // [n_models][arena_cap] padded search tables of the D classes
     int64_t cap, arena_cap;
-    int Jpad, n_groups, B, n_models, n_tiles, seg_cap;
+    int Jpad, n_groups, B, n_models, n_tiles, seg_cap, mts;   // mts: table stride per realisation (1, or 0 in repeat mode)
     int64_t P;
     uint32_t key0, key1, model0;
     float *part;             // [n_models][seg_cap][B][P]
@@ -275,12 +275,13 @@ __global__ void __launch_bounds__(S2_THREADS, S2_MINB) k_stage2(const S2Args a) 
         const int sg = unit % a.seg_cap;
         const int rem = unit / a.seg_cap;
         const int m = rem / a.n_tiles, tile = rem - m * a.n_tiles;
-        const SegTable *seg = a.seg + m;
+        const int mt = m * a.mts;                        // whose tables realisation m reads
+        const SegTable *seg = a.seg + mt;
         if (sg >= seg->n_seg) continue;
         const int g_lo = seg->g_lo[sg], g_hi = seg->g_hi[sg], cls = seg->cls[sg];
-        const GroupRec *grp = a.grp + (size_t)m * a.n_groups;
-        const PointRec *rec = a.rec + (size_t)m * a.Jpad;
-        const uint32_t *tab = a.tab + (size_t)m * a.cap;
+        const GroupRec *grp = a.grp + (size_t)mt * a.n_groups;
+        const PointRec *rec = a.rec + (size_t)mt * a.Jpad;
+        const uint32_t *tab = a.tab + (size_t)mt * a.cap;
         const uint32_t mctr = a.model0 + (uint32_t)m;
         uint32_t pix[S2_PX];
 #pragma unroll
@@ -288,7 +289,7 @@ __global__ void __launch_bounds__(S2_THREADS, S2_MINB) k_stage2(const S2Args a) 
         st.reset();
         const int D = cls == S2_CLS_D9 ? 9 : (cls == S2_CLS_D7 ? 7 : (cls == S2_CLS_D5 ? 5 : 0));
         const int csz = D ? (S2_TABW >> (D + 2)) : S2_CHUNK;       // groups per chunk
-        const uint32_t *xsrc = a.arena + (size_t)m * a.arena_cap + seg->arena_off[cls];
+        const uint32_t *xsrc = a.arena + (size_t)mt * a.arena_cap + seg->arena_off[cls];
         const int cls0 = seg->cls_start[cls];
         const int n_chunks = (g_hi - g_lo + csz - 1) / csz;
         auto stage = [&](int c, int buf) {      // thread 0: bulk copies (TMA) of chunk c into buffer buf
@@ -350,7 +351,7 @@ __global__ void __launch_bounds__(S2_THREADS, S2_MINB) k_stage2(const S2Args a) 
 struct RdArgs {
     const float *part; const SegTable *seg; const DevModel *mdl;
     float *flux_raw, *flux_dust;
-    int B, seg_cap, dust_mode, n_models;
+    int B, seg_cap, dust_mode, n_models, mts;
     int64_t P;
     uint32_t key0, key1, model0;
     double dust_frac, coef[4];
@@ -361,10 +362,10 @@ __global__ void __launch_bounds__(256) k_reduce_dust(const RdArgs a) {
     if (idx >= a.P * a.n_models) return;
     const int m = (int)(idx / a.P);
     const uint32_t p = (uint32_t)(idx - (int64_t)m * a.P);
-    const int n_seg = a.seg[m].n_seg;
+    const int n_seg = a.seg[m * a.mts].n_seg;
     float A = 0.f; bool behind = true;
     if (a.dust_mode != 0) {       // fp32: the factor needs 1e-5 relative, expf / exp10f give 1e-7
-        const DevModel M = a.mdl[m];
+        const DevModel M = a.mdl[m * a.mts];
         uint32_t w[4];
         philox4x32_10(a.key0, a.key1, p, 0u, a.model0 + (uint32_t)m, 1u, w);
         A = (float)M.dust_med * expf((float)M.dust_sigma * normal_f32(w[0], w[1]));
@@ -410,7 +411,7 @@ int pcmd_launch_stage2(pcmd_ctx *c, int n_models, uint64_t seed, uint32_t model0
     a.grp = c->d_grp; a.seg = c->d_seg; a.rec = c->d_rec; a.tab = c->d_tab; a.mult = c->d_mult;
     a.arena = c->d_arena; a.arena_cap = c->arena_cap;
     a.cap = c->cap_raw; a.Jpad = c->Jpad; a.n_groups = c->Jpad >> 2; a.B = c->B; a.n_models = n_models;
-    a.n_tiles = (int)((c->P + S2_TILE - 1) / S2_TILE); a.seg_cap = c->seg_cap; a.P = c->P;
+    a.n_tiles = (int)((c->P + S2_TILE - 1) / S2_TILE); a.seg_cap = c->seg_cap; a.P = c->P; a.mts = c->tab_stride;
     a.key0 = (uint32_t)(seed & 0xFFFFFFFFull); a.key1 = (uint32_t)(seed >> 32); a.model0 = model0;
     a.part = c->d_part; a.hash = d_hash; a.total = d_total; a.counter = c->d_status + 1;
     if (d_hash) {
@@ -430,7 +431,7 @@ int pcmd_launch_stage2(pcmd_ctx *c, int n_models, uint64_t seed, uint32_t model0
 
     RdArgs r;
     r.part = c->d_part; r.seg = c->d_seg; r.mdl = c->d_model; r.flux_raw = d_flux_raw; r.flux_dust = c->d_fdust;
-    r.B = c->B; r.seg_cap = c->seg_cap; r.dust_mode = c->dust_mode; r.n_models = n_models; r.P = c->P;
+    r.mts = c->tab_stride; r.B = c->B; r.seg_cap = c->seg_cap; r.dust_mode = c->dust_mode; r.n_models = n_models; r.P = c->P;
     r.key0 = a.key0; r.key1 = a.key1; r.model0 = model0; r.dust_frac = c->dust_frac;
     for (int b = 0; b < 4; ++b) r.coef[b] = c->dust_coef[b];
     const int64_t n = c->P * n_models;
