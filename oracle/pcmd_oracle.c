@@ -329,12 +329,20 @@ int orc_stage3(const orc_config *c, const orc_params *p, uint64_t seed, uint32_t
 int orc_stage4(const orc_config *c, const double *F_in, double *G) {
     const int B = c->n_bands, N = c->n_im, K = c->psf_k, r = (K - 1) / 2;
     const int64_t P = (int64_t)N * N;
+    /* PAPER.md:180 "we subdivide each image into a 4 x 4 grid and apply to each a different PSF
+     * convolution, shifted by fractions of a pixel" (DESIGN.md R-Q19): cells of ceil(N/G) pixels; the
+     * output pixel (y, x) uses the PSF of its cell; the sum runs over the whole (circular) image. */
+    const int Gd = c->psf_grid > 1 ? c->psf_grid : 1;
+    const int cell = (N + Gd - 1) / Gd;
     for (int b = 0; b < B; ++b) {
-        const double *psf = c->psf + (size_t)b * K * K;
         const double *F = F_in + (size_t)b * P;
 #pragma omp parallel for
         for (int y = 0; y < N; ++y)
             for (int x = 0; x < N; ++x) {
+                int gy = y / cell, gx = x / cell;
+                if (gy > Gd - 1) gy = Gd - 1;
+                if (gx > Gd - 1) gx = Gd - 1;
+                const double *psf = c->psf + ((size_t)b * Gd * Gd + (size_t)gy * Gd + gx) * K * K;
                 double s = 0.0;
                 for (int dy = -r; dy <= r; ++dy)
                     for (int dx = -r; dx <= r; ++dx) {

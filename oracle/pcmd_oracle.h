@@ -43,6 +43,9 @@ typedef struct {
     double         dust_frac;    /* F_dust                        */
     int32_t        dust_mode;    /* 0 none, 1 star fraction, 2 pixel mixture     */
     double         mdf_cut;      /* 0.01                          */
+    int32_t        psf_grid;     /* G: 0/1 one PSF per band; G > 1: psf is [B][G*G][K][K], the image is
+                                    divided into a G x G grid of cells and an output pixel uses the PSF
+                                    of its cell (DESIGN.md R-Q19)  */
 } orc_config;
 
 /* One model = the paper's free parameters (Table 1). */

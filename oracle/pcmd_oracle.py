@@ -41,7 +41,8 @@ class _Config(C.Structure):
                 ("dust_coef", C.c_void_p), ("psf", C.c_void_p), ("psf_k", C.c_int32),
                 ("sky", C.c_void_p), ("read_sigma", C.c_void_p),
                 ("shot_noise", C.c_int32), ("poisson_sky", C.c_int32),
-                ("dust_frac", C.c_double), ("dust_mode", C.c_int32), ("mdf_cut", C.c_double)]
+                ("dust_frac", C.c_double), ("dust_mode", C.c_int32), ("mdf_cut", C.c_double),
+                ("psf_grid", C.c_int32)]
 
 
 class _Params(C.Structure):
@@ -160,15 +161,20 @@ class Oracle:
         k["feh_idx"] = np.ascontiguousarray(wl["feh_idx"], dtype=np.int32)
         for name in ("imf_w", "absmag", "feh_grid", "zp", "dust_coef", "sky", "read_sigma"):
             k[name] = np.ascontiguousarray(wl[name], dtype=np.float64)
-        k["psf"] = np.ascontiguousarray(wl["psf2d"], dtype=np.float64)  # [B][K][K]
-        assert k["psf"].shape == (self.B, wl["psf_k"], wl["psf_k"])
+        G = int(wl.get("psf_grid", 1) or 1)
+        if G > 1:
+            k["psf"] = np.ascontiguousarray(wl["psf_grid2d"], dtype=np.float64)  # [B][G*G][K][K]
+            assert k["psf"].shape == (self.B, G * G, wl["psf_k"], wl["psf_k"])
+        else:
+            k["psf"] = np.ascontiguousarray(wl["psf2d"], dtype=np.float64)  # [B][K][K]
+            assert k["psf"].shape == (self.B, wl["psf_k"], wl["psf_k"])
         assert k["absmag"].shape == (self.J, self.B)
         self.cfg = _Config(self.N, self.B, self.A, self.Z, self.J,
                            _p(k["age_idx"]), _p(k["feh_idx"]), _p(k["imf_w"]), _p(k["absmag"]),
                            _p(k["feh_grid"]), _p(k["zp"]), _p(k["dust_coef"]), _p(k["psf"]),
                            int(wl["psf_k"]), _p(k["sky"]), _p(k["read_sigma"]),
                            int(wl["shot_noise"]), int(wl["poisson_sky"]), float(wl["dust_frac"]),
-                           int(wl["dust_mode"]), float(wl["mdf_cut"]))
+                           int(wl["dust_mode"]), float(wl["mdf_cut"]), G)
 
     def _params(self, prm: dict):
         sfh = np.ascontiguousarray(prm["sfh"], dtype=np.float64)

@@ -404,3 +404,48 @@ def test_loglike_is_stochastic_and_tightens_with_nim():
         sc.append(np.std(ll))
         assert len(set(ll)) == 8
     assert sc[1] < sc[0]
+
+
+# ---- sub-pixel PSF grid (DESIGN.md R-Q19) ------------------------------------------
+def test_psf_grid_with_identical_psfs_equals_the_single_psf():
+    wl = W.scaled(W.config(2), 20)
+    G = 4
+    g = dict(wl, psf_grid=G, psf_grid2d=np.repeat(wl["psf2d"][:, None], G * G, axis=1))
+    rng = np.random.default_rng(5)
+    F = rng.uniform(1.0, 100.0, size=(wl["n_bands"], 400))
+    assert np.array_equal(O.Oracle(g).stage4(F), O.Oracle(wl).stage4(F))
+
+
+def test_psf_grid_of_shifted_deltas_shifts_every_cell_by_its_own_offset():
+    """Each cell's PSF is a delta at a different whole-pixel offset: the output pixel (y, x) of cell c
+    must be the input pixel (y - dy_c, x - dx_c) (circular) -- brute force with numpy indexing."""
+    wl = W.scaled(W.config(2), 10)          # cells of ceil(10/4) = 3 pixels: 3,3,3,1
+    K, B, G, N = int(wl["psf_k"]), int(wl["n_bands"]), 4, 10
+    r = (K - 1) // 2
+    rng = np.random.default_rng(6)
+    offs = rng.integers(-r, r + 1, size=(B, G * G, 2))
+    psf = np.zeros((B, G * G, K, K), dtype=np.float32)
+    for b in range(B):
+        for c in range(G * G):
+            psf[b, c, offs[b, c, 0] + r, offs[b, c, 1] + r] = 1.0
+    F = rng.uniform(1.0, 100.0, size=(B, N * N))
+    got = O.Oracle(dict(wl, psf_grid=G, psf_grid2d=psf)).stage4(F).reshape(B, N, N)
+    cell = -(-N // G)
+    for b in range(B):
+        Fb = F[b].reshape(N, N)
+        for y in range(N):
+            for x in range(N):
+                c = min(G - 1, y // cell) * G + min(G - 1, x // cell)
+                dy, dx = offs[b, c]
+                assert got[b, y, x] == Fb[(y - dy) % N, (x - dx) % N]
+
+
+def test_psf_grid_generator_is_normalised_and_shifted():
+    wl = W.with_psf_grid(W.scaled(W.config(3), 16), 4)
+    p = wl["psf_grid2d"].astype(np.float64)
+    assert p.shape == (3, 16, 15, 15)
+    assert np.allclose(p.sum(axis=(2, 3)), 1.0, atol=1e-6)
+    d = np.arange(-7, 8)
+    cx = (p * d[None, None, None, :]).sum(axis=(2, 3))           # centroid in x per (band, cell)
+    want = (np.arange(4) + 0.5) / 4 - 0.5
+    assert np.allclose(cx[0].reshape(4, 4)[0], want, atol=2e-3)

@@ -227,6 +227,29 @@ def with_psf(wl: dict, psf_k: int, sigmas) -> dict:
     return out
 
 
+def with_psf_grid(wl: dict, G: int = 4) -> dict:
+    """Sub-pixel PSF grid: G x G Gaussian PSFs per band, the one of cell (gy, gx) shifted
+    by ((gx + 0.5) / G - 0.5, (gy + 0.5) / G - 0.5) pixel, each normalised to 1 (fp32)."""
+    out = dict(wl)
+    K, B = int(wl["psf_k"]), int(wl["n_bands"])
+    r = (K - 1) // 2
+    d = np.arange(-r, r + 1, dtype=np.float64)
+    # recover each band's sigma from its 1-D factor: ratio of the two central samples
+    grid = np.empty((B, G * G, K, K), dtype=np.float32)
+    for b in range(B):
+        f = wl["psf1d"][b].astype(np.float64)
+        sigma = 1.0 if K < 3 else float(np.sqrt(0.5 / np.log(f[r] / f[r + 1])))
+        for gy in range(G):
+            for gx in range(G):
+                sx, sy = (gx + 0.5) / G - 0.5, (gy + 0.5) / G - 0.5
+                p = np.exp(-0.5 * (((d[None, :] - sx) / sigma) ** 2 + ((d[:, None] - sy) / sigma) ** 2))
+                grid[b, gy * G + gx] = (p / p.sum()).astype(np.float32)
+    out["psf_grid"] = int(G)
+    out["psf_grid2d"] = grid
+    out["name"] = wl["name"] + "+grid%d" % G
+    return out
+
+
 def tiny_model(n_im=4, J=8, B=2, seed=7, lam_scale=1.0) -> dict:
     """A 4x4-image, J-point, single-isochrone workload for brute-force checks."""
     rng = np.random.default_rng(seed)
