@@ -80,6 +80,10 @@ typedef struct {
     double         dust_frac;   /* F_dust                                         */
     int32_t        dust_mode;   /* 0 none, 1 star fraction, 2 pixel mixture (R-Q7)               */
     double         mdf_cut;     /* 0.01                                           */
+    int32_t        psf_grid;    /* G: 0 or 1: one PSF per band.  2..8: sub-pixel PSF grid (PAPER.md:180,
+                                   R-Q19): psf is [B][G*G][K][K] (psf_separable must be 0), the image is
+                                   divided into G x G cells of ceil(N/G) pixels and an output pixel is
+                                   convolved with the PSF of its cell (index gy*G + gx)              */
 } pcmd_config;
 
 /* One model = the paper's free parameters (Table 1). */

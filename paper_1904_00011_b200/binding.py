@@ -50,7 +50,7 @@ class Config(C.Structure):
                 ("psf_separable", C.c_int32), ("sky", C.c_void_p), ("read_sigma", C.c_void_p),
                 ("shot_noise", C.c_int32), ("poisson_sky", C.c_int32), ("like_floor", C.c_double),
                 ("n_hess", C.c_int32), ("hess", C.c_void_p), ("dust_frac", C.c_double),
-                ("dust_mode", C.c_int32), ("mdf_cut", C.c_double)]
+                ("dust_mode", C.c_int32), ("mdf_cut", C.c_double), ("psf_grid", C.c_int32)]
 
 
 class Params(C.Structure):
@@ -139,7 +139,12 @@ class Pcmd:
         for name in ("imf_w", "absmag", "feh_grid", "zp", "dust_coef", "sky", "read_sigma"):
             k[name] = np.ascontiguousarray(wl[name], dtype=np.float64)
         K = int(wl["psf_k"])
-        if separable:
+        G = int(wl.get("psf_grid", 1) or 1)
+        if G > 1:
+            if separable:
+                raise ValueError("a PSF grid needs psf_separable=0")
+            k["psf"] = np.ascontiguousarray(wl["psf_grid2d"], dtype=np.float32)   # [B][G*G][K][K]
+        elif separable:
             f = np.ascontiguousarray(wl["psf1d"], dtype=np.float32)          # [B][K]
             k["psf"] = np.ascontiguousarray(np.stack([f, f], axis=1))        # [B][2][K]
         else:
@@ -154,7 +159,7 @@ class Pcmd:
                      _np(k["psf"]), K, int(bool(separable)), _np(k["sky"]), _np(k["read_sigma"]),
                      int(wl["shot_noise"]), int(wl["poisson_sky"]), float(wl.get("like_floor", 0.1)),
                      len(self.hess_specs), C.addressof(hs), float(wl["dust_frac"]), int(wl["dust_mode"]),
-                     float(wl["mdf_cut"]))
+                     float(wl["mdf_cut"]), G)
         self._ctx = C.c_void_p()
         rc = lib().pcmd_create(C.byref(self._ctx), C.byref(cfg))
         if rc:

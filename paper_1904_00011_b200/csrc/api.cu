@@ -86,7 +86,8 @@ extern "C" int pcmd_create(pcmd_ctx **out, const pcmd_config *cfg) {
     if (cfg->n_im < 1 || cfg->n_im > 32768 || cfg->n_bands < 1 || cfg->n_bands > PCMD_MAX_BANDS ||
         cfg->n_age < 1 || cfg->n_feh < 1 || cfg->n_points < 1 || cfg->psf_k < 1 || cfg->psf_k > 63 ||
         (cfg->psf_k & 1) == 0 || cfg->n_hess < 0 || cfg->n_hess > PCMD_MAX_HESS ||
-        cfg->dust_mode < 0 || cfg->dust_mode > 2)
+        cfg->dust_mode < 0 || cfg->dust_mode > 2 || cfg->psf_grid < 0 || cfg->psf_grid > 8 ||
+        (cfg->psf_grid > 1 && cfg->psf_separable))
         return PCMD_EINVAL;
     if (!cfg->age_idx || !cfg->feh_idx || !cfg->imf_w || !cfg->absmag || !cfg->feh_grid || !cfg->zp ||
         !cfg->dust_coef || !cfg->psf || !cfg->sky || !cfg->read_sigma || (cfg->n_hess && !cfg->hess))
@@ -139,16 +140,20 @@ extern "C" int pcmd_create(pcmd_ctx **out, const pcmd_config *cfg) {
     TRY(upload(c, &c->d_imf_w, cfg->imf_w, (size_t)J));
     TRY(upload(c, &c->d_absmag, cfg->absmag, (size_t)J * B));
     TRY(upload(c, &c->d_feh_grid, cfg->feh_grid, (size_t)cfg->n_feh));
-    {   // PSF: kept as [B][K][K]; a separable PSF is expanded (column factor (x) row factor)
-        float *p2 = (float *)malloc((size_t)B * K * K * sizeof(float));
+    {   // PSF: kept as [B][G*G][K][K]; a separable PSF is expanded (column factor (x) row factor)
+        const int G2 = cfg->psf_grid > 1 ? cfg->psf_grid * cfg->psf_grid : 1;
+        c->psf_grid = cfg->psf_grid > 1 ? cfg->psf_grid : 1;
+        float *p2 = (float *)malloc((size_t)B * G2 * K * K * sizeof(float));
         if (!p2) { pcmd_destroy(c); return PCMD_ENOMEM; }
-        for (int b = 0; b < B; ++b)
-            for (int y = 0; y < K; ++y)
-                for (int x = 0; x < K; ++x)
-                    p2[((size_t)b * K + y) * K + x] = cfg->psf_separable
-                        ? (float)((double)cfg->psf[((size_t)b * 2 + 1) * K + y] * (double)cfg->psf[((size_t)b * 2) * K + x])
-                        : cfg->psf[((size_t)b * K + y) * K + x];
-        rc = upload(c, &c->d_psf, p2, (size_t)B * K * K);
+        if (G2 > 1) memcpy(p2, cfg->psf, (size_t)B * G2 * K * K * sizeof(float));
+        else
+            for (int b = 0; b < B; ++b)
+                for (int y = 0; y < K; ++y)
+                    for (int x = 0; x < K; ++x)
+                        p2[((size_t)b * K + y) * K + x] = cfg->psf_separable
+                            ? (float)((double)cfg->psf[((size_t)b * 2 + 1) * K + y] * (double)cfg->psf[((size_t)b * 2) * K + x])
+                            : cfg->psf[((size_t)b * K + y) * K + x];
+        rc = upload(c, &c->d_psf, p2, (size_t)B * G2 * K * K);
         free(p2);
         if (rc) { pcmd_destroy(c); return rc; }
         if (cfg->psf_separable) TRY(upload(c, &c->d_psf_sep, cfg->psf, (size_t)B * 2 * K));

@@ -24,7 +24,7 @@ struct CvArgs {
     float *tap_conv;     // optional
     const uint32_t *sky_tab;
     PointRec sky_rec[4];
-    int N, B, K;
+    int N, B, K, G;      // G: PSF grid cells per side (1: one PSF per band)
     int64_t P;
     int shot_noise, poisson_sky;
     uint32_t key0, key1, model0;
@@ -44,24 +44,48 @@ __global__ void __launch_bounds__(CV_TX * CV_ROWS) k_conv_noise(const CvArgs a) 
     const float *F = a.F + (size_t)mb * a.P;
     const int x0 = blockIdx.x * CV_TX, y0 = blockIdx.y * CV_TY;
     const int tid = threadIdx.y * CV_TX + threadIdx.x, nt = CV_TX * CV_ROWS;
-    for (int t = tid; t < K * K; t += nt) spsf[t] = a.psf[(size_t)b * K * K + t];
     for (int i = threadIdx.y; i < TH; i += CV_ROWS) {      // halo tile with circular wrap (R-Q9)
         const float *row = F + (size_t)wrap_index(y0 - r + i, N) * N;
         for (int j = threadIdx.x; j < TW; j += CV_TX) tile[i * TW + j] = row[wrap_index(x0 - r + j, N)];
     }
-    __syncthreads();
     const int lx = threadIdx.x;
     float acc[CV_TY / CV_ROWS];
 #pragma unroll
     for (int q = 0; q < CV_TY / CV_ROWS; ++q) acc[q] = 0.f;
-    for (int ka = 0; ka < K; ++ka)
-        for (int kb = 0; kb < K; ++kb) {
-            const float w = spsf[ka * K + kb];
+    // Sub-pixel PSF grid (R-Q19): G x G cells of `cell` pixels, an output pixel uses its
+    // cell's PSF.  The tile is convolved once per cell it touches (G = 1: once).
+    const int G = a.G, cell = (N + G - 1) / G;
+    const int gy0 = min(G - 1, y0 / cell), gy1 = min(G - 1, min(N - 1, y0 + CV_TY - 1) / cell);
+    const int gx0 = min(G - 1, x0 / cell), gx1 = min(G - 1, min(N - 1, x0 + CV_TX - 1) / cell);
+    const int my_gx = min(G - 1, (x0 + lx) / cell);
+    for (int gy = gy0; gy <= gy1; ++gy)
+        for (int gx = gx0; gx <= gx1; ++gx) {
+            __syncthreads();           // the previous cell's PSF (and, first time, the tile stores) are done
+            for (int t = tid; t < K * K; t += nt) spsf[t] = a.psf[(((size_t)b * G + gy) * G + gx) * K * K + t];
+            __syncthreads();
+            if (my_gx != gx) continue;
+            bool mine[CV_TY / CV_ROWS];
+            bool any = false;
 #pragma unroll
             for (int q = 0; q < CV_TY / CV_ROWS; ++q) {
-                const int ly = threadIdx.y + q * CV_ROWS;
-                acc[q] = fmaf(w, tile[(ly + 2 * r - ka) * TW + (lx + 2 * r - kb)], acc[q]);
+                mine[q] = min(G - 1, (y0 + (int)threadIdx.y + q * CV_ROWS) / cell) == gy;
+                any |= mine[q];
             }
+            if (!any) continue;
+            float part[CV_TY / CV_ROWS];
+#pragma unroll
+            for (int q = 0; q < CV_TY / CV_ROWS; ++q) part[q] = 0.f;
+            for (int ka = 0; ka < K; ++ka)
+                for (int kb = 0; kb < K; ++kb) {
+                    const float w = spsf[ka * K + kb];
+#pragma unroll
+                    for (int q = 0; q < CV_TY / CV_ROWS; ++q) {
+                        const int ly = threadIdx.y + q * CV_ROWS;
+                        part[q] = fmaf(w, tile[(ly + 2 * r - ka) * TW + (lx + 2 * r - kb)], part[q]);
+                    }
+                }
+#pragma unroll
+            for (int q = 0; q < CV_TY / CV_ROWS; ++q) if (mine[q]) acc[q] = part[q];
         }
     noise_mag_epilogue(a, acc, x0, y0, lx, m, b, mb);
 }
@@ -160,7 +184,7 @@ int pcmd_launch_conv_noise(pcmd_ctx *c, int n_models, uint64_t seed, uint32_t mo
         a.sky_rec[b] = c->sky_rec[b];
         a.zp[b] = c->zp[b]; a.sky[b] = c->sky[b]; a.read_sigma[b] = c->read_sigma[b];
     }
-    a.N = c->N; a.B = c->B; a.K = c->K; a.P = c->P;
+    a.N = c->N; a.B = c->B; a.K = c->K; a.G = c->psf_grid; a.P = c->P;
     a.shot_noise = c->shot_noise; a.poisson_sky = c->poisson_sky;
     a.key0 = (uint32_t)(seed & 0xFFFFFFFFull); a.key1 = (uint32_t)(seed >> 32); a.model0 = model0;
     const int K = c->K;

@@ -52,6 +52,7 @@ struct DevModel {          // per-model scalars staged from pcmd_params
 
 struct pcmd_ctx {
     // ---- configuration (host copies)
+    int32_t psf_grid;      // G >= 1 cells per side, PSF table [B][G*G][K][K]
     int32_t N, B, A, Z, J, Jpad, K, psf_sep, shot_noise, poisson_sky, n_hess, dust_mode;
     int64_t P, hess_bins;
     double like_floor, dust_frac, mdf_cut;

@@ -125,3 +125,31 @@ def test_bad_arguments_are_rejected_without_touching_the_device():
     with pytest.raises(G.PcmdError):
         g.simulate([dict(wl["params"][0], sfh=np.array([-1.0]))])
     g.close()
+
+
+@pytest.mark.parametrize("c,n_im,G", [(3, 40, 4), (2, 48, 3), (1, 64, 4), (2, 7, 4)])
+def test_subpixel_psf_grid(c, n_im, G):
+    """PAPER.md:180 (R-Q19): G x G shifted PSFs, an output pixel uses the PSF of its cell; cells that
+    do not line up with the 32 x 32 CUDA tiles, and an image smaller than a cell row."""
+    import torch
+    Gm = _G()
+    wl = W.with_psf_grid(W.scaled(W.config(c), n_im), G)
+    orc = O.Oracle(wl)
+    o = orc.simulate(wl["params"][0], seed=2)
+    g = Gm.Pcmd(wl)
+    fc = torch.empty((1, g.B, g.N, g.N), dtype=torch.float32, device="cuda")
+    g.debug_taps(None, fc)
+    out = g.simulate(wl["params"][:1], seed=2)
+    torch.cuda.synchronize()
+    assert g.status() == 0
+    assert np.allclose(fc.cpu().numpy().reshape(g.B, -1), o["G"], rtol=1e-5, atol=0)
+    mag = out["mag"].cpu().numpy().reshape(g.B, -1)
+    ok = ~np.isnan(o["mag"])
+    assert np.array_equal(np.isnan(mag), ~ok)
+    assert np.max(np.abs(mag[ok] - o["mag"][ok])) <= 1e-5
+    # and it is not the un-shifted PSF's answer
+    o1 = O.Oracle(W.scaled(W.config(c), n_im)).stage4(o["F_dust"])
+    assert not np.allclose(o1, o["G"], rtol=1e-4, atol=0)
+    g.close()
+    with pytest.raises(ValueError):
+        Gm.Pcmd(wl, separable=True)
