@@ -154,6 +154,56 @@ __device__ __forceinline__ void philox4x32_10(uint32_t k0, uint32_t k1, uint32_t
     out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
 }
 
+// The same generator for the stage-2 counter (pixel, group, model, 0), with everything that does
+// not depend on the group taken out of the group loop.  Round 1 multiplies only the pixel and the
+// model; of round 2, M1*c2 is pixel-only and M0*c0 depends on the group alone (one product serves
+// every pixel of the thread); of round 3, M0*c0 is pixel-only.  7 full rounds remain per call.
+struct PhiloxPix {          // per (pixel, model, key): 4 registers
+    uint32_t X;             // lo(M0 pix) ^ (k1 + W1)          -> c2 after round 2 = hi(M0 c0') ^ X
+    uint32_t Y;             // lo(M1 c2') ^ (k0 + 2 W0)        -> c0 after round 3 = hi(M1 c2'') ^ Y
+    uint32_t Z;             // hi(M0 c0'') ^ (k1 + 2 W1)       -> c2 after round 3 = Z ^ lo(M0 c0')
+    uint32_t L3;            // lo(M0 c0'')                     -> c3 after round 3
+};
+struct PhiloxGrp { uint32_t qh, ql; };   // hi, lo of M0 * c0' (c0' = hi(M1 model) ^ group ^ k0)
+
+__device__ __forceinline__ PhiloxPix philox_pix_setup(uint32_t k0, uint32_t k1, uint32_t pix, uint32_t model) {
+    PhiloxPix h;
+    const uint32_t hi0 = __umulhi(PHILOX_M0, pix), lo0 = PHILOX_M0 * pix;     // round 1, c0 = pix
+    const uint32_t lo1 = PHILOX_M1 * model;                                   // round 1, c2 = model
+    const uint32_t c2p = hi0 ^ k1;                                            // c2' (c3 = stream 0)
+    const uint32_t k0b = k0 + PHILOX_W0, k1b = k1 + PHILOX_W1;                // round-2 keys
+    const uint32_t h2 = __umulhi(PHILOX_M1, c2p), l2 = PHILOX_M1 * c2p;       // round 2, pixel-only product
+    const uint32_t c0pp = h2 ^ lo1 ^ k0b;                                     // c0'' (c1' = lo1)
+    const uint32_t k0c = k0b + PHILOX_W0, k1c = k1b + PHILOX_W1;              // round-3 keys
+    h.X = lo0 ^ k1b;
+    h.Y = l2 ^ k0c;
+    h.Z = __umulhi(PHILOX_M0, c0pp) ^ k1c;
+    h.L3 = PHILOX_M0 * c0pp;
+    return h;
+}
+__device__ __forceinline__ PhiloxGrp philox_grp_setup(uint32_t k0, uint32_t model, uint32_t group) {
+    const uint32_t c0p = __umulhi(PHILOX_M1, model) ^ group ^ k0;             // c0' (c1 = group)
+    PhiloxGrp q;
+    q.qh = __umulhi(PHILOX_M0, c0p); q.ql = PHILOX_M0 * c0p;
+    return q;
+}
+__device__ __forceinline__ void philox_stage2(uint32_t k0, uint32_t k1, const PhiloxPix &h, const PhiloxGrp &q,
+                                              uint32_t out[4]) {
+    // state after round 3
+    const uint32_t c2pp = q.qh ^ h.X;                                         // c2''
+    const uint32_t hm = __umulhi(PHILOX_M1, c2pp), lm = PHILOX_M1 * c2pp;     // round 3, the one real product
+    uint32_t c0 = hm ^ h.Y, c1 = lm, c2 = h.Z ^ q.ql, c3 = h.L3;
+    k0 += 3u * PHILOX_W0; k1 += 3u * PHILOX_W1;
+#pragma unroll
+    for (int r = 3; r < 10; ++r) {
+        uint32_t h0 = __umulhi(PHILOX_M0, c0), l0 = PHILOX_M0 * c0;
+        uint32_t h1 = __umulhi(PHILOX_M1, c2), l1 = PHILOX_M1 * c2;
+        c0 = h1 ^ c1 ^ k0; c1 = l1; c2 = h0 ^ c3 ^ k1; c3 = l0;
+        k0 += PHILOX_W0; k1 += PHILOX_W1;
+    }
+    out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+
 // Box-Muller normal from two words (R-C4), fp64: it is O(P) work, not O(P J).
 __device__ __forceinline__ double normal_from_words(uint32_t w0, uint32_t w1) {
     double u1 = ((double)w0 + 0.5) * (1.0 / 4294967296.0);

@@ -286,6 +286,9 @@ __global__ void __launch_bounds__(S2_THREADS, S2_MINB) k_stage2(const S2Args a) 
         uint32_t pix[S2_PX];
 #pragma unroll
         for (int i = 0; i < S2_PX; ++i) pix[i] = (uint32_t)tile * S2_TILE + (uint32_t)i * S2_THREADS + threadIdx.x;
+        PhiloxPix ph[S2_PX];          // the group-independent part of the Philox rounds, per pixel
+#pragma unroll
+        for (int i = 0; i < S2_PX; ++i) ph[i] = philox_pix_setup(a.key0, a.key1, pix[i], mctr);
         st.reset();
         const int D = cls == S2_CLS_D9 ? 9 : (cls == S2_CLS_D7 ? 7 : (cls == S2_CLS_D5 ? 5 : 0));
         const int csz = D ? (S2_TABW >> (D + 2)) : S2_CHUNK;       // groups per chunk
@@ -313,9 +316,9 @@ __global__ void __launch_bounds__(S2_THREADS, S2_MINB) k_stage2(const S2Args a) 
             for (int g = 0; g < ng; ++g) {                                                     \
                 const GroupRec *gr = sb + g;                                                   \
                 uint32_t u[S2_PX][4];                                                          \
-                const uint32_t go = gr->g_orig;                                                \
+                const PhiloxGrp pq = philox_grp_setup(a.key0, mctr, gr->g_orig);               \
                 _Pragma("unroll") for (int i = 0; i < S2_PX; ++i)                              \
-                    philox4x32_10(a.key0, a.key1, pix[i], go, mctr, 0u, u[i]);                 \
+                    philox_stage2(a.key0, a.key1, ph[i], pq, u[i]);                            \
                 BODY;                                                                          \
                 if ((g & (S2_FLUSH - 1)) == S2_FLUSH - 1) st.flush();                          \
             }
