@@ -47,6 +47,9 @@ SM_COUNT, SCHED_PER_SM, LANES = 148, 4, 32
 # measured on this pool's B200 (profiles/README.md): a kernel that does nothing but Philox4x32-10
 # delivers 5.13e11 calls/s = 2.05e12 draws/s (the IMAD.WIDE pipe is the tightest pipe of stage 2)
 PHILOX_CEILING_DRAWS = 2.05e12
+# dram__bytes_read.sum + dram__bytes_write.sum of one k_stage2 launch from the committed `ncu --set full`
+# capture (profiles/r1d_c3_launches_and_stage2.md); only known for the configuration that was profiled
+NCU_TRAFFIC_BYTES = {("c3", 1): 1.32e6 + 2.62e6}
 
 
 def i_alg(n_bands: int) -> int:
@@ -304,7 +307,7 @@ def run_ours(args):
                         "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h)},
                 "roofline": {"kernel": "k_stage2 (Poisson draws -> pixel flux)", "bound": "alu",
                              "achieved": ach, "peak": peak_inst, "unit": "Tinst/s",
-                             "frac": ach / peak_inst, "traffic": None,
+                             "frac": ach / peak_inst, "traffic": NCU_TRAFFIC_BYTES.get(("c%d" % args.config, n)),
                              "frac_of_philox_ceiling": (draws / (s2_ms * 1e-3)) / PHILOX_CEILING_DRAWS if s2_ms > 0 else None,
                              "i_alg_thread_inst_per_draw": ia, "draws_per_launch": draws,
                              "ms_per_launch": s2_ms, "peak_source": which + " sm_max_mhz"}}
