@@ -54,3 +54,32 @@ def test_full_size_config(c, models):
             assert np.array_equal(Hg, H32)
             assert int(Hg.sum()) + int(stn[m, hi]["n_out"]) + int(stn[m, hi]["n_bad"]) == g.P
     g.close()
+
+
+@pytest.mark.parametrize("c", [2, 3, 5])
+def test_full_size_closed_forms(c):
+    """Properties that hold at any size (north_star): over the pixels of a full-size image the raw flux
+    has mean sum(lambda f) and variance sum(lambda f^2) (compound Poisson), and the star count per pixel
+    is Poisson(N_pix): mean = variance = N_pix (footnote 3).  lambda and f from the ORACLE."""
+    import torch
+    import paper_1904_00011_b200 as G
+    wl = W.config(c)
+    g = G.Pcmd(wl, separable=True)
+    prm = wl["params"][0]
+    out = g.simulate([prm], seed=11, want_raw=True, want_counts=True)
+    torch.cuda.synchronize()
+    assert g.status() == 0
+    _, lam, flux = O.Oracle(wl).stage1(prm)
+    F = out["flux_raw"][0].cpu().numpy().reshape(g.B, -1).astype(np.float64)
+    tot = out["total"][0].cpu().numpy().view(np.uint32).astype(np.float64)
+    P = g.P
+    n_pix = lam.sum()
+    assert abs(tot.mean() - n_pix) <= 5 * np.sqrt(n_pix / P)
+    assert abs(tot.var() - n_pix) <= 5 * n_pix * np.sqrt(2.0 / P) + 5 * np.sqrt(n_pix / P)
+    for b in range(g.B):
+        m1, m2 = (lam * flux[:, b]).sum(), (lam * flux[:, b] ** 2).sum()
+        m4 = (lam * flux[:, b] ** 4).sum()
+        assert abs(F[b].mean() - m1) <= 5 * np.sqrt(m2 / P)
+        # variance of the sample variance of a compound Poisson sum: (kappa_4 + 2 sigma^4) / P, kappa_4 = sum(lambda f^4)
+        assert abs(F[b].var() - m2) <= 5 * np.sqrt((m4 + 2 * m2 * m2) / P)
+    g.close()
