@@ -12,7 +12,8 @@ template <bool SMEM>
 __global__ void __launch_bounds__(HS_THREADS) k_hess(const float *__restrict__ mag, int B, int64_t P,
                                                      const DevHess *__restrict__ specs, int n_hess, int64_t ppb,
                                                      int64_t bins_total, uint32_t *__restrict__ hess,
-                                                     pcmd_hess_stats *__restrict__ part) {
+                                                     pcmd_hess_stats *__restrict__ part,
+                                                     pcmd_hess_stats *__restrict__ stats_out) {
     extern __shared__ uint32_t sh[];
     const int h = blockIdx.y, m = blockIdx.z;
     const DevHess S = specs[h];
@@ -43,12 +44,25 @@ __global__ void __launch_bounds__(HS_THREADS) k_hess(const float *__restrict__ m
         const float4 *vp = reinterpret_cast<const float4 *>(mp), *vm = reinterpret_cast<const float4 *>(mm),
                      *vy = reinterpret_cast<const float4 *>(my);
         const int64_t q1 = (p1 + 3) >> 2;
-        for (int64_t q = (p0 >> 2) + threadIdx.x; q < q1; q += HS_THREADS) {
-            const float4 A = vp[q], Bv = vm[q], Y = vy[q];
+        const bool y_is_minus = (my == mm), y_is_plus = (my == mp);    // the usual case: y is one of the colour's bands
+        auto four = [&](int64_t q, const float4 &A, const float4 &Bv, const float4 &Y) {
             one(A.x, Bv.x, Y.x);
             if (4 * q + 1 < p1) one(A.y, Bv.y, Y.y);
             if (4 * q + 2 < p1) one(A.z, Bv.z, Y.z);
             if (4 * q + 3 < p1) one(A.w, Bv.w, Y.w);
+        };
+        int64_t q = (p0 >> 2) + threadIdx.x;
+        for (; q + HS_THREADS < q1; q += 2 * HS_THREADS) {             // two 16-byte loads per band in flight
+            const float4 A0 = vp[q], B0 = vm[q], A1 = vp[q + HS_THREADS], B1 = vm[q + HS_THREADS];
+            const float4 Y0 = y_is_minus ? B0 : (y_is_plus ? A0 : vy[q]);
+            const float4 Y1 = y_is_minus ? B1 : (y_is_plus ? A1 : vy[q + HS_THREADS]);
+            four(q, A0, B0, Y0);
+            four(q + HS_THREADS, A1, B1, Y1);
+        }
+        for (; q < q1; q += HS_THREADS) {
+            const float4 A = vp[q], Bv = vm[q];
+            const float4 Y = y_is_minus ? Bv : (y_is_plus ? A : vy[q]);
+            four(q, A, Bv, Y);
         }
     } else {
         for (int64_t p = p0 + threadIdx.x; p < p1; p += HS_THREADS) one(mp[p], mm[p], my[p]);
@@ -73,12 +87,17 @@ __global__ void __launch_bounds__(HS_THREADS) k_hess(const float *__restrict__ m
             st.n_in += r_n[0][w]; st.n_out += r_n[1][w]; st.n_bad += r_n[2][w];
             st.sum_x += r_sx[w]; st.sum_y += r_sy[w];
         }
-        part[((size_t)m * n_hess + h) * gridDim.x + blockIdx.x] = st;
+        if (gridDim.x == 1 && stats_out) stats_out[(size_t)m * n_hess + h] = st;   // the only block: final stats
+        else part[((size_t)m * n_hess + h) * gridDim.x + blockIdx.x] = st;
     }
     if (SMEM) {
-        for (int t = threadIdx.x; t < nbins; t += HS_THREADS) {
-            uint32_t v = sh[t];
-            if (v) atomicAdd(&gh[t], v);
+        if (gridDim.x == 1) {       // the only block of this diagram: plain stores, no memset needed
+            for (int t = threadIdx.x; t < nbins; t += HS_THREADS) gh[t] = sh[t];
+        } else {
+            for (int t = threadIdx.x; t < nbins; t += HS_THREADS) {
+                uint32_t v = sh[t];
+                if (v) atomicAdd(&gh[t], v);
+            }
         }
     }
 }
@@ -112,7 +131,8 @@ int pcmd_launch_hess(pcmd_ctx *c, const float *d_mag, int n_models, uint32_t *d_
                      pcmd_hess_stats *d_stats, cudaStream_t s) {
     // pixels per block: at least HS_PIX_PER_BLOCK, more when the batch alone fills the GPU (a block
     // zeroes and flushes a whole private histogram, so long pixel runs amortise that)
-    int64_t want_blocks = ((int64_t)c->sm_count * 8 + (int64_t)n_models * c->n_hess - 1) / ((int64_t)n_models * c->n_hess);
+    int64_t want_blocks = ((int64_t)c->sm_count * 8) / ((int64_t)n_models * c->n_hess);
+    if (want_blocks < 1) want_blocks = 1;
     int64_t ppb = (c->P + want_blocks - 1) / want_blocks;
     if (ppb < HS_PIX_PER_BLOCK) ppb = HS_PIX_PER_BLOCK;
     ppb = (ppb + 1023) & ~(int64_t)1023;
@@ -124,10 +144,11 @@ int pcmd_launch_hess(pcmd_ctx *c, const float *d_mag, int n_models, uint32_t *d_
         PCMD_CUDA(c, cudaMalloc(&c->d_hpart, need * sizeof(pcmd_hess_stats)));
         c->hpart_cap = need;
     }
-    PCMD_CUDA(c, cudaMemsetAsync(d_hess, 0, (size_t)n_models * c->hess_bins * sizeof(uint32_t), s));
     int maxbins = 0;
     for (int h = 0; h < c->n_hess; ++h) maxbins = max(maxbins, c->hess[h].nx * c->hess[h].ny);
     size_t smem = (size_t)maxbins * sizeof(uint32_t);
+    if (!(nblk == 1 && smem <= 200 * 1024))    // a single block per diagram stores its histogram itself
+        PCMD_CUDA(c, cudaMemsetAsync(d_hess, 0, (size_t)n_models * c->hess_bins * sizeof(uint32_t), s));
     dim3 grid(nblk, c->n_hess, n_models);
     if (smem <= 200 * 1024) {
         static size_t smem_set = 0;
@@ -136,13 +157,13 @@ int pcmd_launch_hess(pcmd_ctx *c, const float *d_mag, int n_models, uint32_t *d_
             smem_set = smem;
         }
         k_hess<true><<<grid, HS_THREADS, smem, s>>>(d_mag, c->B, c->P, c->d_hess_spec, c->n_hess, ppb,
-                                                    c->hess_bins, d_hess, c->d_hpart);
+                                                    c->hess_bins, d_hess, c->d_hpart, d_stats);
     } else {
         k_hess<false><<<grid, HS_THREADS, 0, s>>>(d_mag, c->B, c->P, c->d_hess_spec, c->n_hess, ppb,
-                                                  c->hess_bins, d_hess, c->d_hpart);
+                                                  c->hess_bins, d_hess, c->d_hpart, d_stats);
     }
     PCMD_LAUNCHED(c);
-    if (d_stats) {
+    if (d_stats && nblk > 1) {
         k_hess_stats<<<n_models * c->n_hess, 32, 0, s>>>(c->d_hpart, nblk, d_stats);
         PCMD_LAUNCHED(c);
     }
