@@ -21,8 +21,13 @@
 #ifndef S2_MINB
 #define S2_MINB 1
 #endif
+#ifndef S2_UNITS_PER_SLOT
+#define S2_UNITS_PER_SLOT 16
+#endif
 #define S2_TILE (S2_THREADS * S2_PX)
-#define S2_CHUNK 32          // groups per staged chunk (32 * 160 B = 5 KB)
+#ifndef S2_CHUNK
+#define S2_CHUNK 48          // groups per staged chunk (48 * 160 B = 7.5 KB; with the 16 KB table stage: 48 KB static)
+#endif
 #define S2_FLUSH 16          // groups between flushes of the fp32 partial sums into fp64
 #define S2_TABW 4096         // words of staged search tables per buffer (16 KB): 32 / 8 / 2 groups of D5 / D7 / D9
 
@@ -395,7 +400,7 @@ __global__ void __launch_bounds__(256) k_reduce_dust(const RdArgs a) {
 int pcmd_stage2_seg_budget(const pcmd_ctx *c, int n_models) {
     const int64_t tiles = (c->P + S2_TILE - 1) / S2_TILE;
     const int64_t slots = (int64_t)c->sm_count * 4;
-    int64_t b = (16 * slots + n_models * tiles - 1) / (n_models * tiles);
+    int64_t b = (S2_UNITS_PER_SLOT * slots + n_models * tiles - 1) / (n_models * tiles);
     if (b < 1) b = 1;
     if (b > S2_SEG_MAX - S2_NCLASS) b = S2_SEG_MAX - S2_NCLASS;
     return (int)b;
