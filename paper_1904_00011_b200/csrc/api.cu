@@ -185,6 +185,7 @@ extern "C" int pcmd_create(pcmd_ctx **out, const pcmd_config *cfg) {
         if (e != cudaSuccess) { c->last_cuda = (int)e; pcmd_destroy(c); return PCMD_ECUDA; }
     }
     TRY(pcmd_build_sky_tables(c));
+    TRY(pcmd_build_lfact(c));
     TRY(pcmd_stage2_occupancy(c));
 #undef TRY
     cudaDeviceSynchronize();
@@ -197,7 +198,7 @@ extern "C" void pcmd_destroy(pcmd_ctx *c) {
     cudaDeviceSynchronize();
     free_scratch(c);
     cudaFree(c->d_age_idx); cudaFree(c->d_feh_idx); cudaFree(c->d_imf_w); cudaFree(c->d_absmag);
-    cudaFree(c->d_feh_grid); cudaFree(c->d_psf); cudaFree(c->d_psf_sep); cudaFree(c->d_mult); cudaFree(c->d_hess_spec);
+    cudaFree(c->d_feh_grid); cudaFree(c->d_psf); cudaFree(c->d_psf_sep); cudaFree(c->d_mult); cudaFree(c->d_lfact); cudaFree(c->d_hess_spec);
     cudaFree(c->d_sky_tab); cudaFree(c->d_status); cudaFree(c->d_hpart); cudaFree(c->d_part); cudaFree(c->d_fdust);
     cudaFree(c->d_mag); cudaFree(c->d_hessbuf); cudaFree(c->d_statbuf); cudaFree(c->d_lnl);
     cudaFree(c->d_hess_data); cudaFree(c->d_data_stats);

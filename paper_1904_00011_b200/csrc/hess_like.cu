@@ -173,6 +173,19 @@ int pcmd_launch_hess(pcmd_ctx *c, const float *d_mag, int n_models, uint32_t *d_
 // ---------------------------------------------------------------------------------------------
 // Stage 7.  One block per model; every reduction is a fixed-order tree (deterministic).
 #define LL_THREADS 1024
+#define LL_LFACT 4096        // ln(d!) = lgamma(d + 1) tabulated for d < LL_LFACT (computed on the device at pcmd_create)
+
+__global__ void k_lfact(double *__restrict__ t) {
+    const int d = blockIdx.x * blockDim.x + threadIdx.x;
+    if (d < LL_LFACT) t[d] = lgamma((double)d + 1.0);
+}
+
+int pcmd_build_lfact(pcmd_ctx *c) {
+    PCMD_CUDA(c, cudaMalloc(&c->d_lfact, LL_LFACT * sizeof(double)));
+    k_lfact<<<LL_LFACT / 256, 256>>>(c->d_lfact);
+    PCMD_LAUNCHED(c);
+    return PCMD_OK;
+}
 
 __device__ double block_sum(double v, double *scratch) {
 #pragma unroll
@@ -192,6 +205,7 @@ __global__ void __launch_bounds__(LL_THREADS) k_loglike(const uint32_t *__restri
                                                         const pcmd_hess_stats *__restrict__ sd_all,
                                                         const DevHess *__restrict__ specs, int n_hess,
                                                         int64_t bins_total, int mode, double m_floor,
+                                                        const double *__restrict__ lfact,
                                                         double *__restrict__ out) {
     __shared__ double scratch[LL_THREADS / 32];
     const int m = blockIdx.x;
@@ -212,7 +226,7 @@ __global__ void __launch_bounds__(LL_THREADS) k_loglike(const uint32_t *__restri
                 const uint32_t d = hd[i], mo = hm[i];
                 if (d == 0 && mo == 0) continue;
                 const double mu = sc * fmax((double)mo, m_floor);
-                L += (double)d * log(mu) - mu - lgamma((double)d + 1.0);
+                L += (double)d * log(mu) - mu - (d < LL_LFACT ? lfact[d] : lgamma((double)d + 1.0));
             }
             L = block_sum(L, scratch);
         } else {
@@ -242,7 +256,7 @@ int pcmd_launch_loglike(pcmd_ctx *c, const uint32_t *d_hm, const pcmd_hess_stats
                         const uint32_t *d_hd, const pcmd_hess_stats *d_sd, int mode, double *d_out,
                         cudaStream_t s) {
     k_loglike<<<n_models, LL_THREADS, 0, s>>>(d_hm, d_sm, d_hd, d_sd, c->d_hess_spec, c->n_hess,
-                                              c->hess_bins, mode, c->like_floor, d_out);
+                                              c->hess_bins, mode, c->like_floor, c->d_lfact, d_out);
     PCMD_LAUNCHED(c);
     return PCMD_OK;
 }

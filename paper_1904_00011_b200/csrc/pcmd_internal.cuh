@@ -65,6 +65,7 @@ struct pcmd_ctx {
     float *d_psf;          // [B][K][K] (a separable PSF expanded)
     float *d_psf_sep;      // [B][2][K] row and column factors of a separable PSF, else NULL
     uint64_t *d_mult;      // [Jpad] splitmix64(j)|1
+    double *d_lfact;       // ln(d!) table of the Poisson lnL
     DevHess *d_hess_spec;  // [n_hess]
     uint32_t *d_sky_tab;   // [B][sky_cap] stored thresholds minus 1 of Poisson(sky_b)
     PointRec sky_rec[PCMD_MAX_BANDS]; uint32_t sky_cap;
@@ -243,6 +244,7 @@ __device__ __forceinline__ uint32_t count_below(const uint32_t *__restrict__ T, 
 // launchers implemented in the stage files ---------------------------------------------------
 int pcmd_launch_stage1(pcmd_ctx *c, int n_models, cudaStream_t s);
 int pcmd_build_sky_tables(pcmd_ctx *c);
+int pcmd_build_lfact(pcmd_ctx *c);
 int pcmd_launch_stage2(pcmd_ctx *c, int n_models, uint64_t seed, uint32_t model0, float *d_flux_raw,
                        uint64_t *d_hash, uint32_t *d_total, cudaStream_t s);
 int pcmd_stage2_seg_budget(const pcmd_ctx *c, int n_models);
