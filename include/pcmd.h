@@ -177,8 +177,6 @@ int  pcmd_profile(pcmd_ctx *ctx, int32_t enable);
 int  pcmd_stage_ms(pcmd_ctx *ctx, float *h_ms);
 /* Kernels launched on behalf of this ctx since pcmd_create (bench.py's gpu_launches). */
 int64_t pcmd_launch_count(const pcmd_ctx *ctx);
-/* Stage-2 variant: 0 = default choice; see DESIGN.md "Stage 2".  Returns the previous value. */
-int  pcmd_set_option(pcmd_ctx *ctx, const char *name, int64_t value);
 const char *pcmd_strerror(int code);
 
 #ifdef __cplusplus

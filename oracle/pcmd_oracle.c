@@ -467,6 +467,50 @@ int orc_hess_f32(const orc_hess_spec *h, int64_t n_pix, int32_t n_bands, const f
     return 0;
 }
 
+/* Per-pixel form of the two functions above, for the parity tests: bin[i] = iy*nx + ix of pixel i
+ * (the very statements of orc_hess / orc_hess_f32), -1 outside the window, -2 for a NaN magnitude;
+ * near[i] (optional): bit 0 = x within tol_x of a bin edge, bit 1 = y within tol_y of one
+ * (north_star: "Hess bins may differ only for pixels lying within 1e-5 mag of a bin edge"; a colour
+ * is the difference of two magnitudes, so tol_x = 2 tol_y, DESIGN.md R-Q17).
+ * Pinned by tests/test_oracle_stages.py: the histogram of bin[] is orc_hess's, near != 0 is its edge list. */
+int orc_hess_pixels(const orc_hess_spec *h, int64_t n_pix, int32_t n_bands, const double *mag,
+                    double tol_x, double tol_y, int32_t *bin, uint8_t *near) {
+    (void)n_bands;
+    const double dx = (h->x_hi - h->x_lo) / h->nx, dy = (h->y_hi - h->y_lo) / h->ny;
+    for (int64_t i = 0; i < n_pix; ++i) {
+        double mp = mag[(size_t)h->band_plus * n_pix + i], mm = mag[(size_t)h->band_minus * n_pix + i];
+        double my = mag[(size_t)h->band_y * n_pix + i];
+        if (near) near[i] = 0;
+        if (isnan(mp) || isnan(mm) || isnan(my)) { bin[i] = -2; continue; }
+        double x = mp - mm, y = my;
+        if (near) near[i] = (uint8_t)((near_edge(x, h->x_lo, dx, h->nx, tol_x) ? 1 : 0) |
+                                      (near_edge(y, h->y_lo, dy, h->ny, tol_y) ? 2 : 0));
+        double fx = floor((x - h->x_lo) / dx), fy = floor((y - h->y_lo) / dy);
+        if (fx < 0.0 || fx >= (double)h->nx || fy < 0.0 || fy >= (double)h->ny) { bin[i] = -1; continue; }
+        bin[i] = (int32_t)((size_t)fy * h->nx + (size_t)fx);
+    }
+    return 0;
+}
+
+int orc_hess_pixels_f32(const orc_hess_spec *h, int64_t n_pix, int32_t n_bands, const float *mag, int32_t *bin) {
+    (void)n_bands;
+    const float x_lo = (float)h->x_lo, y_lo = (float)h->y_lo;
+    const float inv_dx = (float)((double)h->nx / (h->x_hi - h->x_lo));
+    const float inv_dy = (float)((double)h->ny / (h->y_hi - h->y_lo));
+    for (int64_t i = 0; i < n_pix; ++i) {
+        float mp = mag[(size_t)h->band_plus * n_pix + i], mm = mag[(size_t)h->band_minus * n_pix + i];
+        float my = mag[(size_t)h->band_y * n_pix + i];
+        if (isnan(mp) || isnan(mm) || isnan(my)) { bin[i] = -2; continue; }
+        volatile float x = mp - mm;
+        volatile float tx0 = x - x_lo, ty0 = my - y_lo;
+        volatile float tx = tx0 * inv_dx, ty = ty0 * inv_dy;
+        float fx = floorf(tx), fy = floorf(ty);
+        if (!(fx >= 0.0f) || !(fx < (float)h->nx) || !(fy >= 0.0f) || !(fy < (float)h->ny)) { bin[i] = -1; continue; }
+        bin[i] = (int32_t)((size_t)fy * h->nx + (size_t)fx);
+    }
+    return 0;
+}
+
 /* ------------------------------------------------------------------------
  * Stage 7.  Poisson lnL of the data Hess given the model Hess scaled to the data's
  * pixel count, with a floor on empty model bins (north_star; PAPER.md:226 explains

@@ -118,6 +118,12 @@ int orc_hess(const orc_hess_spec *h, int64_t n_pix, int32_t n_bands, const doubl
 int orc_hess_f32(const orc_hess_spec *h, int64_t n_pix, int32_t n_bands, const float *mag,
                  uint32_t *hess, orc_hess_stats *st);
 
+/* Per-pixel bin index of orc_hess / orc_hess_f32 (-1 outside the window, -2 NaN) and, for the fp64
+ * form, near[i]: bit 0 = x within tol_x of a bin edge, bit 1 = y within tol_y (NULL: not wanted). */
+int orc_hess_pixels(const orc_hess_spec *h, int64_t n_pix, int32_t n_bands, const double *mag,
+                    double tol_x, double tol_y, int32_t *bin, uint8_t *near);
+int orc_hess_pixels_f32(const orc_hess_spec *h, int64_t n_pix, int32_t n_bands, const float *mag, int32_t *bin);
+
 /* ---- stage 7 log-likelihood ---------------------------------------------- */
 /* Poisson lnL (north_star; DESIGN.md R-Q15). */
 double orc_loglike_poisson(const uint32_t *hess_model, const uint32_t *hess_data, int64_t n_bins,

@@ -93,6 +93,9 @@ def lib():
         L.orc_hess.argtypes = [C.c_void_p, C.c_int64, C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p,
                                C.c_double, C.c_void_p, C.c_void_p, C.c_int64]
         L.orc_hess_f32.argtypes = [C.c_void_p, C.c_int64, C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p]
+        L.orc_hess_pixels.argtypes = [C.c_void_p, C.c_int64, C.c_int32, C.c_void_p, C.c_double, C.c_double,
+                                      C.c_void_p, C.c_void_p]
+        L.orc_hess_pixels_f32.argtypes = [C.c_void_p, C.c_int64, C.c_int32, C.c_void_p, C.c_void_p]
         L.orc_stage1.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
         L.orc_philox4x32_10.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
         _lib = L
@@ -284,6 +287,27 @@ class Oracle:
         st = _HessStats()
         lib().orc_hess_f32(C.byref(sp), n_pix, mag32.shape[0], _p(mag32), _p(H), C.byref(st))
         return H, dict(n_in=st.n_in, n_out=st.n_out, n_bad=st.n_bad, sum_x=st.sum_x, sum_y=st.sum_y)
+
+
+    def hess_pixels(self, h: dict, mag, tol_x=2e-5, tol_y=1e-5):
+        """Per-pixel bin index of the fp64 Hess (-1 outside, -2 NaN) and the near-edge flags
+        (bit 0: colour within tol_x of an edge, bit 1: magnitude within tol_y)."""
+        mag = np.ascontiguousarray(mag, dtype=np.float64)
+        n_pix = mag.shape[1]
+        sp = self._spec(h)
+        b = np.zeros(n_pix, dtype=np.int32)
+        near = np.zeros(n_pix, dtype=np.uint8)
+        lib().orc_hess_pixels(C.byref(sp), n_pix, mag.shape[0], _p(mag), tol_x, tol_y, _p(b), _p(near))
+        return b, near
+
+    def hess_pixels_f32(self, h: dict, mag32):
+        """Per-pixel bin index of the kernel-precision Hess decision (orc_hess_f32)."""
+        mag32 = np.ascontiguousarray(mag32, dtype=np.float32)
+        n_pix = mag32.shape[1]
+        sp = self._spec(h)
+        b = np.zeros(n_pix, dtype=np.int32)
+        lib().orc_hess_pixels_f32(C.byref(sp), n_pix, mag32.shape[0], _p(mag32), _p(b))
+        return b
 
 
 def _stats_struct(s: dict):

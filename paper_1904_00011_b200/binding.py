@@ -89,7 +89,6 @@ def lib():
         L.pcmd_last_cuda_error.argtypes = [vp]
         L.pcmd_launch_count.argtypes = [vp]
         L.pcmd_launch_count.restype = i64
-        L.pcmd_set_option.argtypes = [vp, C.c_char_p, i64]
         L.pcmd_profile.argtypes = [vp, i32]
         L.pcmd_stage_ms.argtypes = [vp, vp]
         _lib = L
@@ -213,20 +212,24 @@ class Pcmd:
             out["hash"], out["total"] = hsh, tot
         return out
 
-    def simulate_repeat(self, prm, n_repeats, seed=0, model_index0=0, want_raw=False, mag=None):
+    def simulate_repeat(self, prm, n_repeats, seed=0, model_index0=0, want_raw=False, want_counts=False, mag=None):
         """n_repeats realisations of one parameter vector (stage 1 once)."""
         t = self.torch
         arr, keep = self._params([prm])
         if mag is None:
             mag = t.empty((n_repeats, self.B, self.N, self.N), dtype=t.float32, device="cuda")
         raw = t.empty_like(mag) if want_raw else None
+        hsh = t.empty((n_repeats, self.P), dtype=t.int64, device="cuda") if want_counts else None
+        tot = t.empty((n_repeats, self.P), dtype=t.int32, device="cuda") if want_counts else None
         rc = lib().pcmd_simulate_repeat(self._ctx, C.addressof(arr), n_repeats, C.c_uint64(seed), model_index0,
-                                        _dp(mag), _dp(raw), None, None, self._stream())
+                                        _dp(mag), _dp(raw), _dp(hsh), _dp(tot), self._stream())
         if rc:
             raise PcmdError(rc, "pcmd_simulate_repeat")
         out = dict(mag=mag)
         if want_raw:
             out["flux_raw"] = raw
+        if want_counts:
+            out["hash"], out["total"] = hsh, tot
         return out
 
     def hess(self, mag, want_stats=True, out=None):
@@ -305,9 +308,6 @@ class Pcmd:
 
     def launch_count(self):
         return int(lib().pcmd_launch_count(self._ctx))
-
-    def set_option(self, name, value):
-        return int(lib().pcmd_set_option(self._ctx, name.encode(), int(value)))
 
     @staticmethod
     def stats_to_numpy(st):

@@ -69,13 +69,14 @@ static int ensure_scratch(pcmd_ctx *c, int n_models, int64_t cap_raw) {
     PCMD_CUDA(c, cudaMalloc(&c->d_gpos, (size_t)nm * (Jp / 4) * sizeof(uint32_t)));
     {   // padded search tables: room for every group in D9 (8 KB), capped at 1 GiB over all models
         int64_t words = (int64_t)(Jp / 4) * 2048, lim = ((int64_t)1 << 28) / nm;
+        lim &= ~(int64_t)31;          // every model's arena starts 128-byte aligned (bulk copies need 16 B)
         if (words > lim) words = lim;
         if (words < (int64_t)(Jp / 4) * 128) words = (int64_t)(Jp / 4) * 128;   // D5 always fits
         c->arena_cap = words;
         PCMD_CUDA(c, cudaMalloc(&c->d_arena, (size_t)nm * words * sizeof(uint32_t)));
     }
     c->h_stage_bytes = (size_t)nm * (c->A * sizeof(double) + sizeof(DevModel));
-    PCMD_CUDA(c, cudaMallocHost(&c->h_stage, c->h_stage_bytes));
+    PCMD_CUDA(c, cudaMallocHost(&c->h_stage, 2 * c->h_stage_bytes));
     c->cap_models = nm; c->cap_raw = cr;
     return PCMD_OK;
 }
@@ -134,6 +135,10 @@ extern "C" int pcmd_create(pcmd_ctx **out, const pcmd_config *cfg) {
     c->h_imf_w = (double *)malloc((size_t)J * sizeof(double));
     if (!c->h_imf_w) { delete c; return PCMD_ENOMEM; }
     memcpy(c->h_imf_w, cfg->imf_w, (size_t)J * sizeof(double));
+    for (int j = 0; j < J; ++j) {
+        c->imf_sqrt_sum += sqrt(cfg->imf_w[j]);
+        if (cfg->imf_w[j] > c->imf_w_max) c->imf_w_max = cfg->imf_w[j];
+    }
 #define TRY(x) do { rc = (x); if (rc) { pcmd_destroy(c); return rc; } } while (0)
     TRY(upload(c, &c->d_age_idx, cfg->age_idx, (size_t)J));
     TRY(upload(c, &c->d_feh_idx, cfg->feh_idx, (size_t)J));
@@ -203,7 +208,7 @@ extern "C" void pcmd_destroy(pcmd_ctx *c) {
     cudaFree(c->d_mag); cudaFree(c->d_hessbuf); cudaFree(c->d_statbuf); cudaFree(c->d_lnl);
     cudaFree(c->d_hess_data); cudaFree(c->d_data_stats);
     if (c->h_pin) cudaFreeHost(c->h_pin);
-    if (c->stage_ev_valid) cudaEventDestroy(c->stage_ev);
+    if (c->stage_ev_valid) { cudaEventDestroy(c->stage_ev[0]); cudaEventDestroy(c->stage_ev[1]); }
     if (c->prof_made) for (int i = 0; i < 8; ++i) cudaEventDestroy(c->prof_ev[i]);
     free(c->h_imf_w);
     delete c;
@@ -230,12 +235,14 @@ static int stage_params(pcmd_ctx *c, const pcmd_params *params, int n_models, in
             if (p.sfh[a] > smax) smax = p.sfh[a];
         }
         double tot = 0.0;
-        for (int j = 0; j < c->J; ++j) {
-            const double lb = smax * c->h_imf_w[j];
-            if (lb > PCMD_LAMBDA_MAX) {
+        if (smax * c->imf_w_max <= PCMD_LAMBDA_MAX) {
+            tot = 20.0 * sqrt(smax) * c->imf_sqrt_sum + 96.0 * c->J;   // sum_j 20 sqrt(smax w_j) + 96
+        } else {
+            for (int j = 0; j < c->J; ++j) {
+                const double lb = smax * c->h_imf_w[j];
                 // the bound may be loose (MDF weight < 1); the kernel raises ERANGE on the true value
-                tot += 20.0 * 2048.0 + 96.0;
-            } else tot += 20.0 * sqrt(lb) + 96.0;
+                tot += (lb > PCMD_LAMBDA_MAX) ? 20.0 * 2048.0 + 96.0 : 20.0 * sqrt(lb) + 96.0;
+            }
         }
         if ((int64_t)tot > cap) cap = (int64_t)tot;
     }
@@ -258,7 +265,10 @@ static int stage_params(pcmd_ctx *c, const pcmd_params *params, int n_models, in
         PCMD_CUDA(c, cudaMalloc(&c->d_part, (size_t)need * sizeof(float)));
         c->part_elems = need;
     }
-    double *hs = c->h_stage;
+    // the half of the pinned staging area the previous call did not use: wait only for the call before that
+    c->stage_flip ^= 1;
+    if (c->stage_ev_valid) PCMD_CUDA(c, cudaEventSynchronize(c->stage_ev[c->stage_flip]));
+    double *hs = reinterpret_cast<double *>(reinterpret_cast<char *>(c->h_stage) + (size_t)c->stage_flip * c->h_stage_bytes);
     DevModel *hm = reinterpret_cast<DevModel *>(hs + (size_t)n_models * c->A);
     for (int i = 0; i < n_models; ++i) {
         memcpy(hs + (size_t)i * c->A, params[i].sfh, c->A * sizeof(double));
@@ -276,15 +286,16 @@ static int simulate_impl(pcmd_ctx *c, const pcmd_params *params, int32_t n_model
     if (!c || !params || n_models < 1 || n_real < 1 || !d_mag) return PCMD_EINVAL;
     if ((d_count_hash == nullptr) != (d_count_total == nullptr)) return PCMD_EINVAL;
     cudaStream_t s = (cudaStream_t)cuda_stream;
-    // the pinned staging buffer is reused: wait until the previous call's copies have run
-    if (c->stage_ev_valid) PCMD_CUDA(c, cudaEventSynchronize(c->stage_ev));
-    int rc = stage_params(c, params, n_models, n_real, s);
-    if (rc) return rc;
     if (!c->stage_ev_valid) {
-        PCMD_CUDA(c, cudaEventCreateWithFlags(&c->stage_ev, cudaEventDisableTiming));
+        PCMD_CUDA(c, cudaEventCreateWithFlags(&c->stage_ev[0], cudaEventDisableTiming));
+        PCMD_CUDA(c, cudaEventCreateWithFlags(&c->stage_ev[1], cudaEventDisableTiming));
+        PCMD_CUDA(c, cudaEventRecord(c->stage_ev[0], s));
+        PCMD_CUDA(c, cudaEventRecord(c->stage_ev[1], s));
         c->stage_ev_valid = 1;
     }
-    PCMD_CUDA(c, cudaEventRecord(c->stage_ev, s));
+    int rc = stage_params(c, params, n_models, n_real, s);
+    if (rc) return rc;
+    PCMD_CUDA(c, cudaEventRecord(c->stage_ev[c->stage_flip], s));
     PCMD_CUDA(c, cudaMemsetAsync(c->d_status, 0, 2 * sizeof(int32_t), s));
     c->last_models = n_models;
     c->tab_stride = (n_models == n_real) ? 1 : 0;     // 0: every realisation reads model 0's tables
@@ -454,14 +465,16 @@ __global__ void k_debug_philox(uint32_t k0, uint32_t k1, const uint32_t *__restr
 extern "C" int pcmd_debug_philox(uint64_t seed, const uint32_t *h_ctr, int64_t n, uint32_t *h_out) {
     if (!h_ctr || !h_out || n < 1) return PCMD_EINVAL;
     uint32_t *d_c = nullptr, *d_o = nullptr;
-    pcmd_ctx *none = nullptr;
-    PCMD_CUDA(none, cudaMalloc(&d_c, (size_t)n * 16));
-    PCMD_CUDA(none, cudaMalloc(&d_o, (size_t)n * 16));
-    PCMD_CUDA(none, cudaMemcpy(d_c, h_ctr, (size_t)n * 16, cudaMemcpyHostToDevice));
-    k_debug_philox<<<(unsigned)((n + 127) / 128), 128>>>((uint32_t)(seed & 0xFFFFFFFFull), (uint32_t)(seed >> 32), d_c, n, d_o);
-    PCMD_CUDA(none, cudaGetLastError());
-    PCMD_CUDA(none, cudaMemcpy(h_out, d_o, (size_t)n * 16, cudaMemcpyDeviceToHost));
-    cudaFree(d_c); cudaFree(d_o);
+    cudaError_t e = cudaMalloc(&d_c, (size_t)n * 16);
+    if (e == cudaSuccess) e = cudaMalloc(&d_o, (size_t)n * 16);
+    if (e == cudaSuccess) e = cudaMemcpy(d_c, h_ctr, (size_t)n * 16, cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) {
+        k_debug_philox<<<(unsigned)((n + 127) / 128), 128>>>((uint32_t)(seed & 0xFFFFFFFFull), (uint32_t)(seed >> 32), d_c, n, d_o);
+        e = cudaGetLastError();
+    }
+    if (e == cudaSuccess) e = cudaMemcpy(h_out, d_o, (size_t)n * 16, cudaMemcpyDeviceToHost);
+    cudaFree(d_c); cudaFree(d_o);      // freed on every path
+    if (e != cudaSuccess) return e == cudaErrorMemoryAllocation ? PCMD_ENOMEM : PCMD_ECUDA;
     return PCMD_OK;
 }
 
@@ -499,9 +512,3 @@ extern "C" int pcmd_stage_ms(pcmd_ctx *c, float *h_ms) {
 
 extern "C" int pcmd_last_cuda_error(const pcmd_ctx *c) { return c ? c->last_cuda : 0; }
 extern "C" int64_t pcmd_launch_count(const pcmd_ctx *c) { return c ? c->launches : 0; }
-
-extern "C" int pcmd_set_option(pcmd_ctx *c, const char *name, int64_t value) {
-    if (!c || !name) return PCMD_EINVAL;
-    if (strcmp(name, "stage2") == 0) { int64_t old = c->opt_stage2; c->opt_stage2 = value; return (int)old; }
-    return PCMD_EINVAL;
-}

@@ -197,19 +197,17 @@ int pcmd_launch_conv_noise(pcmd_ctx *c, int n_models, uint64_t seed, uint32_t mo
         else if (K == 15) k_conv_noise_sep<15><<<grid, blk, smem, s>>>(a);
         else if (K == 21) k_conv_noise_sep<21><<<grid, blk, smem, s>>>(a);
         else {
-            static size_t smem_set_sep = 0;
-            if (smem > 48 * 1024 && smem > smem_set_sep) {
+            if (smem > 48 * 1024 && smem > c->smem_conv_sep) {
                 PCMD_CUDA(c, cudaFuncSetAttribute(k_conv_noise_sep<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-                smem_set_sep = smem;
+                c->smem_conv_sep = smem;
             }
             k_conv_noise_sep<0><<<grid, blk, smem, s>>>(a);
         }
     } else {
         size_t smem = ((size_t)(CV_TX + K - 1) * (CV_TY + K - 1) + (size_t)K * K) * sizeof(float);
-        static size_t smem_set = 0;
-        if (smem > 48 * 1024 && smem > smem_set) {
+        if (smem > 48 * 1024 && smem > c->smem_conv) {
             PCMD_CUDA(c, cudaFuncSetAttribute(k_conv_noise, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-            smem_set = smem;
+            c->smem_conv = smem;
         }
         k_conv_noise<<<grid, dim3(CV_TX, CV_ROWS), smem, s>>>(a);
     }

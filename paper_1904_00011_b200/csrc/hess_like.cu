@@ -40,7 +40,7 @@ __global__ void __launch_bounds__(HS_THREADS) k_hess(const float *__restrict__ m
         if (SMEM) atomicAdd(&sh[bin], 1u); else atomicAdd(&gh[bin], 1u);
         n_in++; sx += (double)x; sy += (double)y;
     };
-    if (((P | p0) & 3) == 0) {      // 16-byte loads: every row of every image starts 16-byte aligned
+    if (((P | p0) & 3) == 0 && (reinterpret_cast<uintptr_t>(mag) & 15) == 0) {      // 16-byte loads: every band of every image starts 16-byte aligned
         const float4 *vp = reinterpret_cast<const float4 *>(mp), *vm = reinterpret_cast<const float4 *>(mm),
                      *vy = reinterpret_cast<const float4 *>(my);
         const int64_t q1 = (p1 + 3) >> 2;
@@ -151,10 +151,9 @@ int pcmd_launch_hess(pcmd_ctx *c, const float *d_mag, int n_models, uint32_t *d_
         PCMD_CUDA(c, cudaMemsetAsync(d_hess, 0, (size_t)n_models * c->hess_bins * sizeof(uint32_t), s));
     dim3 grid(nblk, c->n_hess, n_models);
     if (smem <= 200 * 1024) {
-        static size_t smem_set = 0;
-        if (smem > 48 * 1024 && smem > smem_set) {
+        if (smem > 48 * 1024 && smem > c->smem_hess) {
             PCMD_CUDA(c, cudaFuncSetAttribute(k_hess<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-            smem_set = smem;
+            c->smem_hess = smem;
         }
         k_hess<true><<<grid, HS_THREADS, smem, s>>>(d_mag, c->B, c->P, c->d_hess_spec, c->n_hess, ppb,
                                                     c->hess_bins, d_hess, c->d_hpart, d_stats);

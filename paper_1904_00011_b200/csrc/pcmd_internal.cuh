@@ -59,6 +59,7 @@ struct pcmd_ctx {
     double zp[PCMD_MAX_BANDS], dust_coef[PCMD_MAX_BANDS], sky[PCMD_MAX_BANDS], read_sigma[PCMD_MAX_BANDS];
     pcmd_hess_spec hess[PCMD_MAX_HESS];
     double *h_imf_w;       // [J] host copy, used only to size scratch
+    double imf_sqrt_sum, imf_w_max;   // sum_j sqrt(imf_w_j), max_j imf_w_j (scratch sizing)
     // ---- device constants
     int32_t *d_age_idx, *d_feh_idx;
     double *d_imf_w, *d_absmag, *d_feh_grid;
@@ -74,8 +75,9 @@ struct pcmd_ctx {
     int64_t cap_raw;       // entries of raw table scratch per model
     double *d_sfh;         // [cap_models][A]
     DevModel *d_model;     // [cap_models]
-    double *h_stage;       // pinned staging for sfh + DevModel
-    size_t h_stage_bytes;
+    double *h_stage;       // pinned staging for sfh + DevModel: two halves used alternately
+    size_t h_stage_bytes;  // bytes of one half
+    int stage_flip;
     double *d_mdfw;        // [cap_models][Z]
     double *d_lambda;      // [cap_models][J]
     uint32_t *d_rawcnt;    // [cap_models][J+1] raw table range sizes -> exclusive offsets
@@ -103,12 +105,12 @@ struct pcmd_ctx {
     void *h_pin; size_t h_pin_bytes;
     // taps / options / bookkeeping
     float *tap_dust, *tap_conv;
-    int64_t opt_stage2;
+    size_t smem_conv, smem_conv_sep, smem_hess;   // opted-in dynamic shared memory of this ctx's device
     int32_t last_models;
     int last_cuda;
     int64_t launches;
     int sm_count;
-    cudaEvent_t stage_ev; int stage_ev_valid;
+    cudaEvent_t stage_ev[2]; int stage_ev_valid;
     // per-stage timing (pcmd_profile): events recorded on the caller's stream around each stage
     cudaEvent_t prof_ev[8]; int prof_on, prof_made; uint32_t prof_seen;
 };

@@ -153,3 +153,23 @@ def test_subpixel_psf_grid(c, n_im, G):
     g.close()
     with pytest.raises(ValueError):
         Gm.Pcmd(wl, separable=True)
+
+
+def test_capped_arena_non_power_of_two_batch():
+    """50 <= n_models < 799 at J = 10 500 caps the per-model arena of padded search tables at 2^28 / n_models
+    words; every model's arena must still start 16-byte aligned for the bulk copies (a batch that is not a
+    power of two used to leave model 1 misaligned).  All models against the oracle."""
+    wl = W.scaled(W.config(4), 32)
+    base = wl["params"]
+    prms = [base[i % len(base)] for i in range(50)]
+    # make some models D-class heavy so that the arena is really read
+    for i in (1, 7, 49):
+        prms[i] = dict(prms[i], sfh=np.asarray(prms[i]["sfh"]) * 40.0)
+    r = _run(wl, prms, seed=5, separable=True)
+    assert r["status"] == 0
+    orc = O.Oracle(wl)
+    for i in (0, 1, 7, 23, 49):
+        o = orc.simulate(prms[i], seed=5, model=i)
+        assert np.array_equal(r["total"][i], o["total"]) and np.array_equal(r["hash"][i], o["hash"])
+        assert np.allclose(r["raw"][i], o["F_raw"], rtol=1e-5, atol=0)
+    r["g"].close()

@@ -1,58 +1,72 @@
 """Parity at BASELINE.json's full sizes, in the launch configuration bench.py times (separable PSF,
-production kernels).  Stage 2 (the Monte Carlo part): sampled pixels, which the oracle computes one
-by one -- counts bit-exact, flux 1e-5.  Stages 3-5: the oracle run on the GPU's own raw flux
-(stage-isolated, every pixel).  Stage 6: exact in the kernel's precision; counts add up."""
+production kernels), against the fp64 oracle run on the WHOLE image end to end: every pixel of every
+stage, the Hess per-pixel edge rule and the log-likelihood (tests/_parity.py states the rules)."""
 import numpy as np
 import pytest
 
 from oracle import pcmd_oracle as O
 from workloads import synthetic as W
+from _parity import EDGE_TOL_X, EDGE_TOL_Y, FLUX_RTOL, MAG_ATOL, hess_pixel_parity, lnl_poisson_parity
 
 pytestmark = pytest.mark.gpu
 
 
 @pytest.mark.parametrize("c,models", [(2, [0]), (3, [0]), (4, [0, 17, 63]), (5, [0])])
 def test_full_size_config(c, models):
+    """Whole image, every pixel, against the fp64 oracle run end to end (PAPER.md:71,81,83 stages 1-5, :218
+    stage 6, north_star stage 7): counts bit-exact, raw / dusty / convolved flux 1e-5 relative, magnitudes
+    1e-5 mag, Hess per-pixel edge-membership rule, lnL 1e-4."""
     import torch
     import paper_1904_00011_b200 as G
     wl = W.config(c)
     seed = int(wl["seed"])
     g = G.Pcmd(wl, separable=True)
     prms = wl["params"]
+    n = len(prms)
     out = g.simulate(prms, seed=seed, want_raw=True, want_counts=True)
-    fast = g.simulate(prms, seed=seed, want_raw=True)                  # production kernel
+    fd = torch.empty((n, g.B, g.N, g.N), dtype=torch.float32, device="cuda")
+    fc = torch.empty_like(fd)
+    g.debug_taps(fd, fc)
+    fast = g.simulate(prms, seed=seed, want_raw=True)                  # production kernel, as bench.py runs it
+    g.debug_taps(None, None)
     H, st = g.hess(fast["mag"])
+    data = np.concatenate([d.ravel() for d in wl["data_hess"]]).astype(np.uint32)
+    lnl = g.loglike(H, st, torch.from_numpy(data.view(np.int32)).cuda()).cpu().numpy()
     torch.cuda.synchronize()
     assert g.status() == 0
     assert torch.equal(out["flux_raw"], fast["flux_raw"])
+    assert torch.equal(out["mag"].view(torch.int32), fast["mag"].view(torch.int32))
     orc = O.Oracle(wl)
-    rng = np.random.default_rng(1234 + c)
-    pix = np.unique(np.concatenate([rng.integers(0, g.P, 1500), [0, g.N - 1, g.P - g.N, g.P - 1]])).astype(np.uint32)
     stn = G.Pcmd.stats_to_numpy(st)
     for m in models:
-        mdfw, lam, flux = orc.stage1(prms[m])
+        o = orc.simulate(prms[m], seed=seed, model=m)                  # the whole image
         w = g.debug_weights(m)
-        assert np.array_equal(w["lam"], lam)
-        F, tot, hsh = orc.stage2(lam, flux, seed, model=m, pix=pix)
-        assert np.array_equal(out["total"][m].cpu().numpy().view(np.uint32)[pix], tot)
-        assert np.array_equal(out["hash"][m].cpu().numpy().view(np.uint64)[pix], hsh)
+        assert np.array_equal(w["lam"], o["lam"])
+        assert np.array_equal(out["total"][m].cpu().numpy().view(np.uint32), o["total"])      # every pixel
+        assert np.array_equal(out["hash"][m].cpu().numpy().view(np.uint64), o["hash"])
         raw = fast["flux_raw"][m].cpu().numpy().reshape(g.B, -1)
-        assert np.allclose(raw[:, pix], F, rtol=1e-5, atol=0)
-        # stages 3-5 on the GPU's raw flux
-        _, Fd = orc.stage3(prms[m], raw.astype(np.float64), seed, model=m)
-        mag_o = orc.stage5(orc.stage4(Fd), seed, model=m)
+        assert np.allclose(raw, o["F_raw"], rtol=FLUX_RTOL, atol=0)
+        assert np.allclose(fd[m].cpu().numpy().reshape(g.B, -1), o["F_dust"], rtol=FLUX_RTOL, atol=0)
+        assert np.allclose(fc[m].cpu().numpy().reshape(g.B, -1), o["G"], rtol=FLUX_RTOL, atol=0)
         mag = fast["mag"][m].cpu().numpy().reshape(g.B, -1)
-        ok = ~np.isnan(mag_o)
+        ok = ~np.isnan(o["mag"])
         assert np.array_equal(np.isnan(mag), ~ok)
-        assert np.max(np.abs(mag[ok] - mag_o[ok])) <= 1e-5
-        off = 0
+        dmag = float(np.max(np.abs(mag[ok] - o["mag"][ok])))
+        assert dmag <= MAG_ATOL
+        off, parts = 0, []
         for hi, h in enumerate(wl["hess"]):
             nb = h["nx"] * h["ny"]
-            Hg = H[m].cpu().numpy().view(np.uint32)[off:off + nb].reshape(h["ny"], h["nx"])
+            Hg = H[m].cpu().numpy().view(np.uint32)[off:off + nb]
             off += nb
-            H32, s32 = orc.hess_f32(h, mag)
-            assert np.array_equal(Hg, H32)
-            assert int(Hg.sum()) + int(stn[m, hi]["n_out"]) + int(stn[m, hi]["n_bad"]) == g.P
+            moved, b64, b32, H64, s64 = hess_pixel_parity(orc, h, mag, o["mag"], Hg)
+            parts.append((H64, b64, b32, moved))
+            sg = stn[m, hi]
+            assert int(Hg.sum()) + int(sg["n_out"]) + int(sg["n_bad"]) == g.P
+            assert int(sg["n_bad"]) == s64["n_bad"]
+            print("[c%d model %d hess %d] max |dmag| %.2e; %d of %d pixels moved bin, all within (%g, %g) mag of "
+                  "an edge (oracle n_edge at 1e-5: %d)" % (c, m, hi, dmag, moved.size, g.P, EDGE_TOL_X, EDGE_TOL_Y,
+                                                            s64["n_edge"]))
+        lnl_poisson_parity(float(lnl[m]), parts, data, wl["like_floor"], "c%d model %d" % (c, m))
     g.close()
 
 

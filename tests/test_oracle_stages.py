@@ -347,6 +347,46 @@ def test_hess_f32_agrees_with_f64_away_from_edges(c1):
     assert s32["n_in"] + s32["n_out"] + s32["n_bad"] == P
 
 
+def test_hess_pixels_is_the_per_pixel_form_of_hess(c1):
+    """orc_hess_pixels / orc_hess_pixels_f32 (used by the GPU parity tests for the per-pixel edge-membership
+    check) against orc_hess / orc_hess_f32 and against plain numpy floor arithmetic."""
+    rng = np.random.default_rng(12)
+    P = 30000
+    m1 = rng.uniform(17, 31, P)
+    m0 = m1 + rng.normal(1.0, 1.2, P)
+    m0[::101] = np.nan
+    # a few pixels a hair away from an edge on either axis
+    m1[5], m0[5] = 20.0 + 6e-6, 20.0 + 6e-6 + 0.55
+    m1[6], m0[6] = 22.3, 22.3 + 1.0 - 1.5e-5          # x within 2e-5, not within 1e-5
+    mag = np.stack([m0, m1])
+    h = _hspec(40, 60)     # dx = 0.1, dy = 0.2
+    o = O.Oracle(c1)
+    H, st = o.hess(h, mag, edge_tol=1e-5, want_edges=True)
+    b, near = o.hess_pixels(h, mag, tol_x=1e-5, tol_y=1e-5)
+    assert np.array_equal(np.bincount(b[b >= 0], minlength=h["nx"] * h["ny"]).reshape(h["ny"], h["nx"]), H)
+    assert (b == -2).sum() == st["n_bad"] and (b == -1).sum() == st["n_out"]
+    assert np.array_equal(np.nonzero(near)[0].astype(np.uint32), st["edges"])
+    assert near[5] == 2 and near[6] == 0
+    _, near2 = o.hess_pixels(h, mag, tol_x=2e-5, tol_y=1e-5)
+    assert near2[6] == 1 and np.all((near2 & 2) == (near & 2)) and np.all(near2 >= near)
+    # plain numpy definition of the bin index
+    ok = ~np.isnan(m0)
+    ix = np.floor(((m0 - m1) - h["x_lo"]) / ((h["x_hi"] - h["x_lo"]) / h["nx"]))
+    iy = np.floor((m1 - h["y_lo"]) / ((h["y_hi"] - h["y_lo"]) / h["ny"]))
+    inw = ok & (ix >= 0) & (ix < h["nx"]) & (iy >= 0) & (iy < h["ny"])
+    assert np.array_equal(b[inw], (iy[inw] * h["nx"] + ix[inw]).astype(np.int32))
+    assert np.all(b[ok & ~inw] == -1)
+    # fp32 form
+    mag32 = mag.astype(np.float32)
+    H32, s32 = o.hess_f32(h, mag32)
+    b32 = o.hess_pixels_f32(h, mag32)
+    assert np.array_equal(np.bincount(b32[b32 >= 0], minlength=h["nx"] * h["ny"]).reshape(h["ny"], h["nx"]), H32)
+    assert (b32 == -2).sum() == s32["n_bad"] and (b32 == -1).sum() == s32["n_out"]
+    # away from edges both precisions agree pixel by pixel
+    b64, near64 = o.hess_pixels(h, mag32.astype(np.float64), tol_x=2e-5, tol_y=1e-5)
+    assert np.all((b32 == b64) | (near64 != 0))
+
+
 # ------------------------------------------------------------------ stage 7
 def test_loglike_poisson_vs_scipy():
     rng = np.random.default_rng(10)
