@@ -35,9 +35,9 @@ extern "C" const char *pcmd_strerror(int code) {
 static void free_scratch(pcmd_ctx *c) {
     cudaFree(c->d_sfh); cudaFree(c->d_model); cudaFree(c->d_mdfw); cudaFree(c->d_lambda);
     cudaFree(c->d_rawcnt); cudaFree(c->d_klo); cudaFree(c->d_q); cudaFree(c->d_stcnt);
-    cudaFree(c->d_tab); cudaFree(c->d_rec); cudaFree(c->d_grp); cudaFree(c->d_seg);
+    cudaFree(c->d_tab); cudaFree(c->d_rec); cudaFree(c->d_grp); cudaFree(c->d_plan);
     cudaFree(c->d_gcls); cudaFree(c->d_arena); cudaFree(c->d_gpos);
-    c->d_grp = nullptr; c->d_seg = nullptr; c->d_gcls = nullptr; c->d_arena = nullptr; c->d_gpos = nullptr;
+    c->d_grp = nullptr; c->d_plan = nullptr; c->d_gcls = nullptr; c->d_arena = nullptr; c->d_gpos = nullptr;
     if (c->h_stage) cudaFreeHost(c->h_stage);
     c->d_sfh = nullptr; c->d_model = nullptr; c->d_mdfw = nullptr; c->d_lambda = nullptr;
     c->d_rawcnt = nullptr; c->d_klo = nullptr; c->d_q = nullptr; c->d_stcnt = nullptr;
@@ -64,7 +64,7 @@ static int ensure_scratch(pcmd_ctx *c, int n_models, int64_t cap_raw) {
     PCMD_CUDA(c, cudaMalloc(&c->d_tab, (size_t)nm * cr * sizeof(uint32_t)));
     PCMD_CUDA(c, cudaMalloc(&c->d_rec, (size_t)nm * Jp * sizeof(PointRec)));
     PCMD_CUDA(c, cudaMalloc(&c->d_grp, (size_t)nm * (Jp / 4) * sizeof(GroupRec)));
-    PCMD_CUDA(c, cudaMalloc(&c->d_seg, (size_t)nm * sizeof(SegTable)));
+    PCMD_CUDA(c, cudaMalloc(&c->d_plan, (size_t)nm * sizeof(ModelPlan)));
     PCMD_CUDA(c, cudaMalloc(&c->d_gcls, (size_t)nm * (Jp / 4)));
     PCMD_CUDA(c, cudaMalloc(&c->d_gpos, (size_t)nm * (Jp / 4) * sizeof(uint32_t)));
     {   // padded search tables: room for every group in D9 (8 KB), capped at 1 GiB over all models
@@ -249,8 +249,7 @@ static int stage_params(pcmd_ctx *c, const pcmd_params *params, int n_models, in
     if (cap > 0xFFFFFFF0ll) return PCMD_ERANGE;
     int rc = ensure_scratch(c, n_models, cap);
     if (rc) return rc;
-    c->seg_budget = pcmd_stage2_seg_budget(c, n_real);
-    c->seg_cap = c->seg_budget + S2_NCLASS;
+    c->n_seg = pcmd_stage2_segments(c, n_real);
     const int64_t need_img = (int64_t)n_real * c->B * c->P;
     if (need_img > c->fdust_elems) {
         cudaDeviceSynchronize();
@@ -258,7 +257,7 @@ static int stage_params(pcmd_ctx *c, const pcmd_params *params, int n_models, in
         PCMD_CUDA(c, cudaMalloc(&c->d_fdust, (size_t)need_img * sizeof(float)));
         c->fdust_elems = need_img;
     }
-    const int64_t need = (int64_t)n_real * c->seg_cap * c->B * c->P;
+    const int64_t need = (int64_t)n_real * c->n_seg * c->B * c->P;
     if (need > c->part_elems) {
         cudaDeviceSynchronize();
         cudaFree(c->d_part); c->d_part = nullptr; c->part_elems = 0;

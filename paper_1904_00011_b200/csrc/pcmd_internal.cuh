@@ -17,7 +17,9 @@ struct __align__(16) PointRec {
 
 // Stage-2 work layout.  Groups of four consecutive isochrone points (one
 // Philox call, R-C1) are classified by how many sampler thresholds decide almost every draw and
-// sorted by class; a class is cut into segments; one (model, pixel tile, segment) is a work unit.
+// sorted by class; a class is cut into chunks (the unit of shared-memory staging); the chunks of all
+// (model, pixel tile) pairs form one cost-weighted sequence that is cut into equal shares, one per
+// persistent CTA (no work queue, no atomics).
 #define S2_NCLASS 8        // classes, most expensive first:
 #define S2_CLS_D9 1        //   0 bisection in global memory (tables longer than 511)
 #define S2_CLS_D7 2        //   1-3 branch-free search of a padded table of 2^D words in shared memory
@@ -27,17 +29,37 @@ struct __align__(16) PointRec {
 #define S2_CLS_L1 6
 #define S2_CLS_L0 7        //   7 rare: P(any star) < 2^-8 per draw: one max-compare per group, then class L1's path
 #define S2_CLS_NONE 8      //   no point of the group can have a star: dropped
-#define S2_SEG_MAX 48      // segments per model (all classes together)
+#define S2_CHUNK 48         // group records per staged chunk (48 * 160 B = 7.5 KB)
+#define S2_TABW 4096        // words of staged search tables per chunk (16 KB): 32 / 8 / 2 groups of D5 / D7 / D9
+// cost model of the static partition: ~SM cycles per warp and group of each class loop (profiles/), and per chunk
+#define S2_COST_G 1500u
+#define S2_COST_D9 420u
+#define S2_COST_D7 340u
+#define S2_COST_D5 250u
+#define S2_COST_L4 190u
+#define S2_COST_L2 160u
+#define S2_COST_L1 155u
+#define S2_COST_L0 150u
+#define S2_COST_CHUNK 100u
 struct __align__(16) GroupRec {      // 160 bytes
     uint32_t g_orig, cls, tmin, pad1; // original group index (Philox counter word 1), class, min over w of T[0][w]
-    uint32_t T[5][4];                 // T[i][w]: (i+1)-th stored threshold minus 1 of point w; 0xFFFFFFFF if none
+    uint32_t T[5][4];                 // T[i][w]: (i+1)-th stored threshold minus 1 of point w; 0xFFFFFFFF if none.
+                                      // Search classes D5/D7/D9: T[4][w] = float bits of (float)k0
     float f[4][4];                    // f[w][b]: flux of one star of point w in band b
 };
-struct SegTable {                     // per model
-    int32_t n_seg, pad;
-    int32_t g_lo[S2_SEG_MAX], g_hi[S2_SEG_MAX], cls[S2_SEG_MAX];  // sorted-group ranges
-    int32_t cls_start[S2_NCLASS + 1], first_d;                    // class ranges; first D class kept in the arena
-    int64_t arena_off[S2_NCLASS];                                 // word offset of a class's padded tables
+// Per model: the class-sorted group list cut into chunks.  Chunk i of class c (chunk_start[c] <= i <
+// chunk_start[c+1]) holds groups cls_start[c] + (i - chunk_start[c]) * chunk_groups[c] ... (at most
+// chunk_groups[c] of them) and starts at cost position cost_start[c] + (i - chunk_start[c]) * chunk_cost[c].
+struct __align__(16) ModelPlan {
+    int32_t n_chunks, first_d;                    // first D class whose padded tables are in the arena
+    uint32_t cost_total, cost_max;                // cost of one pixel tile of this model; largest chunk cost
+    int32_t cls_start[S2_NCLASS + 1];             // sorted-group range of each class
+    int32_t chunk_start[S2_NCLASS + 1];           // chunk range of each class
+    uint32_t cost_start[S2_NCLASS + 1];           // cost position of each class's first chunk
+    int32_t chunk_groups[S2_NCLASS];              // groups per full chunk
+    uint32_t chunk_cost[S2_NCLASS];               // cost of a full chunk
+    int32_t run_cls[S2_NCLASS];                   // the loop that runs a class (0 for a D class demoted to bisection)
+    int64_t arena_off[S2_NCLASS];                 // word offset of a class's padded tables in the model's arena
 };
 
 struct DevHess {
@@ -89,12 +111,12 @@ struct pcmd_ctx {
     float *d_fdust; int64_t fdust_elems;   // [realisations][B][P] dusty flux
     int32_t tab_stride;    // 1: realisation m reads model m's tables; 0: all read model 0's (repeat mode)
     GroupRec *d_grp;       // [cap_models][Jpad/4] class-sorted group records
-    SegTable *d_seg;       // [cap_models]
+    ModelPlan *d_plan;     // [cap_models]
     uint8_t *d_gcls;       // [cap_models][Jpad/4] class of each group (original order)
     uint32_t *d_gpos;      // [cap_models][Jpad/4] sorted position of each group
     uint32_t *d_arena; int64_t arena_cap;  // [cap_models][arena_cap] padded search tables of the D classes
-    float *d_part;  int64_t part_elems;  // stage-2 partial fluxes [cap_models][seg_cap][B][P]
-    int32_t seg_budget, seg_cap, s2_ctas_per_sm;
+    float *d_part;  int64_t part_elems;  // stage-2 partial fluxes [realisations][n_seg][B][P]
+    int32_t n_seg, s2_ctas_per_sm;
     int32_t *d_status;     // device status word
     // hess / loglike scratch
     pcmd_hess_stats *d_hpart; int64_t hpart_cap; // per-block partial stats
@@ -249,7 +271,8 @@ int pcmd_build_sky_tables(pcmd_ctx *c);
 int pcmd_build_lfact(pcmd_ctx *c);
 int pcmd_launch_stage2(pcmd_ctx *c, int n_models, uint64_t seed, uint32_t model0, float *d_flux_raw,
                        uint64_t *d_hash, uint32_t *d_total, cudaStream_t s);
-int pcmd_stage2_seg_budget(const pcmd_ctx *c, int n_models);
+int pcmd_stage2_segments(const pcmd_ctx *c, int n_models);
+int pcmd_stage2_tiles(const pcmd_ctx *c);
 int pcmd_stage2_occupancy(pcmd_ctx *c);
 int pcmd_launch_conv_noise(pcmd_ctx *c, int n_models, uint64_t seed, uint32_t model0, float *d_mag,
                            cudaStream_t s);

@@ -244,11 +244,16 @@ __global__ void __launch_bounds__(256) k_group_classify(const PointRec *__restri
     cls_all[(size_t)m * n_groups + g] = (uint8_t)cls;
 }
 
-// Stable counting sort of the groups by class (positions only), segment table, arena layout.
+// Stable counting sort of the groups by class (positions only), chunk layout, arena layout.
 // One block per model.
-__global__ void __launch_bounds__(1024) k_group_sort(const uint8_t *__restrict__ cls_all, int Jpad, int seg_budget,
+//
+// Cost model of stage 2 (cost units ~ SM cycles per warp and group, measured per class loop with
+// ncu, profiles/): the static partition of the chunk sequence among the persistent CTAs is by cost.
+__constant__ uint32_t c_s2_group_cost[S2_NCLASS] = {S2_COST_G, S2_COST_D9, S2_COST_D7, S2_COST_D5,
+                                                    S2_COST_L4, S2_COST_L2, S2_COST_L1, S2_COST_L0};
+__global__ void __launch_bounds__(1024) k_group_sort(const uint8_t *__restrict__ cls_all, int Jpad,
                                                      int64_t arena_cap, uint32_t *__restrict__ pos_all,
-                                                     SegTable *__restrict__ seg_all) {
+                                                     ModelPlan *__restrict__ plan_all) {
     __shared__ uint32_t wcnt[32][S2_NCLASS];
     __shared__ uint32_t count[S2_NCLASS + 1], carry[S2_NCLASS], cls_start[S2_NCLASS + 1];
     const int m = blockIdx.x, n_groups = Jpad >> 2;
@@ -287,9 +292,9 @@ __global__ void __launch_bounds__(1024) k_group_sort(const uint8_t *__restrict__
         __syncthreads();
     }
     if (threadIdx.x == 0) {
-        SegTable t;
+        ModelPlan t;
         // padded search tables: D9 first, then D7, D5; a class that does not fit the arena is
-        // demoted to class 0 (the classes are adjacent in the sorted order, so this is a relabel)
+        // demoted to bisection in global memory (run_cls = 0)
         const int64_t stride[4] = {0, 4 << 9, 4 << 7, 4 << 5};
         int first_d = S2_CLS_D9;
         for (;;) {
@@ -299,36 +304,30 @@ __global__ void __launch_bounds__(1024) k_group_sort(const uint8_t *__restrict__
             first_d++;
         }
         int64_t off = 0;
+        int32_t chunks = 0;
+        uint32_t cost = 0, cmax = 0;
         for (int c = 0; c < S2_NCLASS; ++c) {
             t.cls_start[c] = (int32_t)cls_start[c];
             t.arena_off[c] = 0;
-            if (c >= first_d && c <= S2_CLS_D5) { t.arena_off[c] = off; off += stride[c] * (int64_t)count[c]; }
+            const bool in_arena = c >= first_d && c <= S2_CLS_D5;
+            if (in_arena) { t.arena_off[c] = off; off += stride[c] * (int64_t)count[c]; }
+            const bool demoted = c >= S2_CLS_D9 && c <= S2_CLS_D5 && !in_arena;
+            t.run_cls[c] = demoted ? 0 : c;
+            const int cg = in_arena ? (int)(S2_TABW / stride[c]) : S2_CHUNK;     // groups per chunk
+            t.chunk_groups[c] = cg;
+            t.chunk_cost[c] = (uint32_t)cg * c_s2_group_cost[t.run_cls[c]] + S2_COST_CHUNK;
+            const int n = (int)count[c], nch = (n + cg - 1) / cg;
+            t.chunk_start[c] = chunks;
+            t.cost_start[c] = cost;
+            chunks += nch;
+            cost += (uint32_t)nch * t.chunk_cost[c];     // the last (ragged) chunk is charged as a full one
+            if (nch > 0 && t.chunk_cost[c] > cmax) cmax = t.chunk_cost[c];
         }
         t.cls_start[S2_NCLASS] = (int32_t)cls_start[S2_NCLASS];
-        t.first_d = first_d;
-        // segments: each class gets a share of seg_budget proportional to its estimated cost
-        const float wgt[S2_NCLASS] = {8.0f, 3.2f, 2.6f, 2.0f, 1.5f, 1.15f, 1.0f, 0.8f};
-        float total = 0.f;
-        for (int c = 0; c < S2_NCLASS; ++c) {
-            const float wc = (c >= 1 && c < first_d) ? wgt[0] : wgt[c];
-            total += wc * (float)count[c];
-        }
-        t.n_seg = 0;
-        for (int c = 0; c < S2_NCLASS; ++c) {
-            const int n = (int)count[c];
-            if (n == 0) continue;
-            const float wc = (c >= 1 && c < first_d) ? wgt[0] : wgt[c];
-            int k = (int)(wc * (float)n / total * (float)seg_budget + 0.5f);
-            k = max(1, min(k, n));
-            for (int i = 0; i < k && t.n_seg < S2_SEG_MAX; ++i) {
-                t.g_lo[t.n_seg] = (int)cls_start[c] + (int)((int64_t)n * i / k);
-                t.g_hi[t.n_seg] = (int)cls_start[c] + (int)((int64_t)n * (i + 1) / k);
-                t.cls[t.n_seg] = (c >= 1 && c < first_d) ? 0 : c;
-                t.n_seg++;
-            }
-        }
-        for (int i = t.n_seg; i < S2_SEG_MAX; ++i) { t.g_lo[i] = t.g_hi[i] = 0; t.cls[i] = 0; }
-        seg_all[m] = t;
+        t.chunk_start[S2_NCLASS] = chunks;
+        t.cost_start[S2_NCLASS] = cost;
+        t.n_chunks = chunks; t.first_d = first_d; t.cost_total = cost; t.cost_max = cmax;
+        plan_all[m] = t;
     }
 }
 
@@ -339,7 +338,7 @@ __global__ void __launch_bounds__(256) k_group_emit(const PointRec *__restrict__
                                                     const uint32_t *__restrict__ tab_all, int64_t cap, int Jpad,
                                                     const uint8_t *__restrict__ cls_all,
                                                     const uint32_t *__restrict__ pos_all,
-                                                    const SegTable *__restrict__ seg_all, GroupRec *__restrict__ grp_all,
+                                                    const ModelPlan *__restrict__ plan_all, GroupRec *__restrict__ grp_all,
                                                     uint32_t *__restrict__ arena_all, int64_t arena_cap) {
     const int m = blockIdx.y, n_groups = Jpad >> 2, lane = threadIdx.x & 31;
     const int g = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
@@ -359,11 +358,21 @@ __global__ void __launch_bounds__(256) k_group_emit(const PointRec *__restrict__
         if (w == 0) { o->g_orig = (uint32_t)g; o->cls = (uint32_t)cls; o->tmin = tmin; o->pad1 = 0; }
 #pragma unroll
         for (int i = 0; i < 5; ++i) o->T[i][w] = ((uint32_t)i < r.len) ? tab[r.off + i] : 0xFFFFFFFFu;
-        if (cls <= S2_CLS_D5) o->T[4][w] = r.k0;     // the search classes keep k0 here
+        if (cls <= S2_CLS_D5) {
+            // the search classes keep the first count here: k0 (bisection class), or, for a class whose padded
+            // tables are staged in shared memory, the float k0 - (word offset of the point's table in its
+            // chunk's stage buffer): stage 2 then gets the count from the ADDRESS of the found entry
+            const ModelPlan *pl = plan_all + m;
+            if (cls >= pl->first_d) {
+                const int D = cls == S2_CLS_D9 ? 9 : (cls == S2_CLS_D7 ? 7 : 5);
+                const int g_local = ((int)pos - pl->cls_start[cls]) % pl->chunk_groups[cls];
+                o->T[4][w] = __float_as_uint((float)((int)r.k0 - ((g_local * 4 + w) << D)));
+            } else o->T[4][w] = r.k0;
+        }
 #pragma unroll
         for (int b = 0; b < 4; ++b) o->f[w][b] = r.f[b];
     }
-    const SegTable *t = seg_all + m;
+    const ModelPlan *t = plan_all + m;
     if (cls >= t->first_d && cls <= S2_CLS_D5) {
         const int D = cls == S2_CLS_D9 ? 9 : (cls == S2_CLS_D7 ? 7 : 5);
         uint32_t *dst = arena_all + (size_t)m * arena_cap + t->arena_off[cls] +
@@ -406,10 +415,10 @@ int pcmd_launch_stage1(pcmd_ctx *c, int n_models, cudaStream_t s) {
     k_group_classify<<<dim3((n_groups + 255) / 256, n_models), 256, 0, s>>>(c->d_rec, c->d_tab, c->cap_raw, c->Jpad,
                                                                            c->d_gcls);
     PCMD_LAUNCHED(c);
-    k_group_sort<<<n_models, 1024, 0, s>>>(c->d_gcls, c->Jpad, c->seg_budget, c->arena_cap, c->d_gpos, c->d_seg);
+    k_group_sort<<<n_models, 1024, 0, s>>>(c->d_gcls, c->Jpad, c->arena_cap, c->d_gpos, c->d_plan);
     PCMD_LAUNCHED(c);
     k_group_emit<<<dim3((n_groups + 7) / 8, n_models), 256, 0, s>>>(c->d_rec, c->d_tab, c->cap_raw, c->Jpad, c->d_gcls,
-                                                                    c->d_gpos, c->d_seg, c->d_grp, c->d_arena,
+                                                                    c->d_gpos, c->d_plan, c->d_grp, c->d_arena,
                                                                     c->arena_cap);
     PCMD_LAUNCHED(c);
     return PCMD_OK;
