@@ -111,6 +111,12 @@ __device__ __forceinline__ void sts128(bool lead, void *p, int4 v) {
     asm volatile("{\n.reg .pred q;\nsetp.ne.b32 q, %5, 0;\n@q st.shared.v4.b32 [%0], {%1, %2, %3, %4};\n}"
                  ::"r"(smem_u32(p)), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w), "r"((int)lead) : "memory");
 }
+// volatile load that the compiler may not move other memory accesses across (spin on a flag another warp sets)
+__device__ __forceinline__ uint32_t lds_acquire_u32(const void *p) {
+    uint32_t v;
+    asm volatile("ld.volatile.shared.u32 %0, [%1];" : "=r"(v) : "r"(smem_u32(p)) : "memory");
+    return v;
+}
 __device__ __forceinline__ uint32_t lds_u32(uint32_t addr) {
     uint32_t v;
     asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(addr));
@@ -338,7 +344,8 @@ struct S2Shared {
     ModelPlan plan;                      // the plan of model plan_m (the producer's current model)
     int32_t m_, tile, seg, chunk;        // current unit (model, tile, segment); next chunk to issue
     int32_t chunk_end, cls, live, issued;// end of the unit's chunk range; class of `chunk`; more to issue; chunks issued so far
-    int32_t plan_m, unit_first, pad[2];  // model of `plan`; the next chunk issued starts a unit
+    int32_t plan_m, unit_first, unit_next, ticket;  // model of `plan`; the next chunk issued starts a unit; the unit fetched
+                                          // one step ahead; producer turns completed
 };
 
 // First chunk of plan p whose cost start is >= q; n_chunks if there is none.
@@ -360,16 +367,18 @@ __device__ __forceinline__ int s2_model_segments(const ModelPlan &p, int n_seg) 
     return (int)min((uint32_t)n_seg, max(k, 1u));
 }
 
-// Thread 0: make `unit` (and the ones the counter hands out after it) the current unit; unit_next holds the
-// unit fetched one step ahead, so the latency of the atomic is never waited for.
-__device__ __forceinline__ void s2_advance(const S2Args &a, S2Shared &sh, int &unit_next, bool lead) {
+// Producer warp: make sh.unit_next (or the first valid unit the counter hands out after it) the current unit
+// and fetch the one after it.
+__device__ __forceinline__ void s2_advance(const S2Args &a, S2Shared &sh, bool lead) {
     const int n_units = a.n_models * a.n_tiles * a.n_seg;
     for (;;) {
-        const int u = unit_next;
+        const int u = sh.unit_next;
         if (u >= n_units) { sts32(lead, &sh.live, 0); __syncwarp(); return; }
         int nx = 0;
         if (lead) nx = atomicAdd(a.counter, 1);
-        unit_next = (int)gridDim.x + __shfl_sync(0xffffffffu, nx, 0);
+        __syncwarp();
+        sts32(lead, &sh.unit_next, (int)gridDim.x + __shfl_sync(0xffffffffu, nx, 0));
+        __syncwarp();
         const int seg = u % a.n_seg, r = u / a.n_seg;
         const int m = r / a.n_tiles, tile = r - m * a.n_tiles;
         if (m != sh.plan_m) {
@@ -397,8 +406,7 @@ __device__ __forceinline__ void s2_advance(const S2Args &a, S2Shared &sh, int &u
 
 // Thread 0: issue the current unit's next chunk into stage s (descriptor + bulk copies) and step to the next
 // chunk of the stream.
-__device__ __forceinline__ void s2_issue(const S2Args &a, S2Shared &sh, GroupRec *sbuf, uint32_t *stab, int s,
-                                         int &unit_next, bool lead) {
+__device__ __forceinline__ void s2_issue(const S2Args &a, S2Shared &sh, GroupRec *sbuf, uint32_t *stab, int s, bool lead) {
     const ModelPlan &p = sh.plan;
     const int m = sh.m_, mt = m * a.mts, cls = sh.cls, chunk = sh.chunk;
     const int li = chunk - p.chunk_start[cls], cg = p.chunk_groups[cls];
@@ -418,7 +426,7 @@ __device__ __forceinline__ void s2_issue(const S2Args &a, S2Shared &sh, GroupRec
     __syncwarp();
     sts32(lead, &sh.issued, issued + 1);
     __syncwarp();
-    if (unit_last) { s2_advance(a, sh, unit_next, lead); sts32(lead, &sh.unit_first, 1); }
+    if (unit_last) { s2_advance(a, sh, lead); sts32(lead, &sh.unit_first, 1); }
     else {
         int c2 = cls;
         while (chunk + 1 >= p.chunk_start[c2 + 1]) c2++;
@@ -443,17 +451,18 @@ __global__ void __launch_bounds__(S2_THREADS, S2_MINB) k_stage2(const S2Args a) 
     const int lane = threadIdx.x & 31;
     const bool lead = lane == 0;
     const bool producer = __all_sync(0xffffffffu, threadIdx.x < 32);     // warp 0, as a warp-uniform predicate
-    int unit_next = 0;                   // warp 0: the unit fetched one step ahead
+    const int wid = __reduce_max_sync(0xffffffffu, threadIdx.x >> 5);    // warp index, warp-uniform
     if (producer) {
         sts32(lead, &sh.plan_m, -1); sts32(lead, &sh.issued, 0); sts32(lead, &sh.live, 0); sts32(lead, &sh.unit_first, 1);
+        sts32(lead, &sh.unit_next, blockIdx.x);      // the first unit is static; the counter hands out the rest
+        sts32(lead, &sh.ticket, 0);
         if (lead) {
             for (int s = 0; s < S2_NST; ++s) { mbar_init(&sh.full[s], 1); mbar_init(&sh.empty[s], S2_WARPS); }
             asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         }
         __syncwarp();
-        unit_next = blockIdx.x;          // the first unit is static; the counter hands out the rest
-        s2_advance(a, sh, unit_next, lead);
-        for (int s = 0; s < S2_NST && sh.live; ++s) s2_issue(a, sh, sbuf, stab, s, unit_next, lead);
+        s2_advance(a, sh, lead);
+        for (int s = 0; s < S2_NST && sh.live; ++s) s2_issue(a, sh, sbuf, stab, s, lead);
         if (sh.issued == 0) {            // nothing for this CTA (tiny job): an empty last chunk ends the stream
             sts128(lead, &sh.desc[0], make_int4(0, 0, S2_CLS_L1, 0));
             sts128(lead, &sh.desc[0].flags, make_int4(S2_F_END, 0, 0, 0));
@@ -464,6 +473,7 @@ __global__ void __launch_bounds__(S2_THREADS, S2_MINB) k_stage2(const S2Args a) 
 #ifdef S2_TIMES
     if (threadIdx.x == 0) { long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); a.times[2 * blockIdx.x] = t; }
     unsigned smid; asm volatile("mov.u32 %0, %%smid;" : "=r"(smid));
+    long long dbg_wait = 0, dbg_prod = 0; const long long dbg_t0 = clock64();
 #endif
     S2State<NB, COUNTS> st;
     uint32_t pix[S2_PX];
@@ -474,7 +484,13 @@ __global__ void __launch_bounds__(S2_THREADS, S2_MINB) k_stage2(const S2Args a) 
     int s = 0, sp = 0;
     uint32_t par = 0, parp = 0;
     for (int q = 0;; ++q) {
+#ifdef S2_TIMES
+        const long long tw0 = clock64();
+#endif
         mbar_wait(&sh.full[s], par);
+#ifdef S2_TIMES
+        dbg_wait += clock64() - tw0;
+#endif
         const ChunkDesc d = sh.desc[s];
         const int mt = d.m * a.mts;
         if (d.flags & S2_F_FIRST) {
@@ -535,13 +551,28 @@ __global__ void __launch_bounds__(S2_THREADS, S2_MINB) k_stage2(const S2Args a) 
         }
         if (d.flags & S2_F_END) {
 #ifdef S2_TIMES
-            if (lane == 0) { long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); a.times[2 * gridDim.x + (blockIdx.x * S2_WARPS + (threadIdx.x >> 5))] = t; if (threadIdx.x == 0) a.times[2 * blockIdx.x + 1] = smid; }
+            if (lane == 0) { long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); const int wi = blockIdx.x * S2_WARPS + (threadIdx.x >> 5); a.times[2 * gridDim.x + wi] = t; a.times[(2 + S2_WARPS) * gridDim.x + 3 * wi] = dbg_wait; a.times[(2 + S2_WARPS) * gridDim.x + 3 * wi + 1] = dbg_prod; a.times[(2 + S2_WARPS) * gridDim.x + 3 * wi + 2] = clock64() - dbg_t0; if (threadIdx.x == 0) a.times[2 * blockIdx.x + 1] = smid; }
 #endif
             break;
         }
-        if (producer && q >= 1 && sh.live) {               // chunk q-1's stage takes chunk q-1+S2_NST
-            mbar_wait(&sh.empty[sp], parp);
-            s2_issue(a, sh, sbuf, stab, sp, unit_next, lead);
+        // Producer turn q (after chunk q >= 1): chunk q-1's stage, which every warp has normally left long ago,
+        // takes chunk q-1+S2_NST.  The turns rotate over the warps (no warp is slowed more than the others, nobody
+        // waits for a producer warp) and run in order (ticket).
+        if (q >= 1 && ((q - 1) & (S2_WARPS - 1)) == wid) {
+#ifdef S2_TIMES
+            const long long tp0 = clock64();
+#endif
+            while (lds_acquire_u32(&sh.ticket) != (uint32_t)(q - 1)) { }
+            __threadfence_block();
+            if (lds_acquire_u32(&sh.live)) {
+                mbar_wait(&sh.empty[sp], parp);
+                s2_issue(a, sh, sbuf, stab, sp, lead);
+            }
+            __threadfence_block();
+            sts32(lead, &sh.ticket, q);
+#ifdef S2_TIMES
+            dbg_prod += clock64() - tp0;
+#endif
         }
         sp = s; parp = par;
         if (++s == S2_NST) { s = 0; par ^= 1u; }
@@ -630,7 +661,7 @@ int pcmd_launch_stage2(pcmd_ctx *c, int n_models, uint64_t seed, uint32_t model0
     const int grid = (int)(n_units < slots ? n_units : slots);
 #ifdef S2_TIMES
     static long long *d_times = nullptr;
-    if (!d_times) cudaMalloc(&d_times, (size_t)grid * (2 + S2_WARPS) * sizeof(long long));
+    if (!d_times) cudaMalloc(&d_times, (size_t)grid * (2 + 4 * S2_WARPS) * sizeof(long long));
     a.times = d_times;
 #endif
     cudaError_t e;
@@ -653,7 +684,7 @@ int pcmd_launch_stage2(pcmd_ctx *c, int n_models, uint64_t seed, uint32_t model0
 #ifdef S2_TIMES
     if (getenv("S2_TIMES_FILE")) {
         cudaStreamSynchronize(s);
-        std::vector<long long> h((size_t)grid * (2 + S2_WARPS));
+        std::vector<long long> h((size_t)grid * (2 + 4 * S2_WARPS));
         cudaMemcpy(h.data(), d_times, h.size() * sizeof(long long), cudaMemcpyDeviceToHost);
         FILE *f = fopen(getenv("S2_TIMES_FILE"), "wb"); fwrite(h.data(), sizeof(long long), h.size(), f); fclose(f);
     }
