@@ -363,6 +363,20 @@ def run_hbm_stages(args):
     g.close()
 
 
+def run_pipes(args):
+    """The pipe table DESIGN.md "Rooflines" quotes: sustained warp-instructions per clock per scheduler of
+    each instruction stream, and the draws/s of a kernel that does nothing but Philox4x32-10."""
+    import torch
+    import paper_1904_00011_b200 as G
+    torch.cuda.set_device(0)
+    rows = G.pipe_bench()
+    philox = [r for r in rows if r["name"].startswith("Philox4x32-10")][0]
+    print(json.dumps({"pipes": [{"stream": r["name"], "warp_instr_per_clk_per_scheduler": round(r["rate"], 4),
+                                 "ms": round(r["ms"], 4)} for r in rows],
+                      "philox_calls_per_s": philox["steps_per_s"], "philox_draws_per_s": 4.0 * philox["steps_per_s"],
+                      "launch": "148 SMs x 2 CTAs x 512 threads, 8 independent chains per thread"}))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -376,8 +390,12 @@ def main():
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--hbm-batch", type=int, default=0,
                     help="instead of the benchmark: HBM fraction of stages 4-6 on this many models (L2-exceeding)")
+    ap.add_argument("--pipes", action="store_true",
+                    help="instead of the benchmark: instruction-pipe micro-benchmarks (pcmd_pipe_bench), one JSON line")
     args = ap.parse_args()
-    if args.hbm_batch > 0:
+    if args.pipes:
+        run_pipes(args)
+    elif args.hbm_batch > 0:
         run_hbm_stages(args)
     elif args.impl == "reference":
         run_reference(args)

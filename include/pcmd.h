@@ -179,6 +179,16 @@ int  pcmd_stage_ms(pcmd_ctx *ctx, float *h_ms);
 int64_t pcmd_launch_count(const pcmd_ctx *ctx);
 const char *pcmd_strerror(int code);
 
+/* Instruction-pipe micro-benchmarks on the current device (measurement support for the stage-2
+ * roofline of DESIGN.md "Rooflines"; nothing of the method runs here).  Test `test` (0 <=
+ * test < n, pcmd_pipe_bench_name(test) != NULL) runs `iters` iterations of an unrolled stream of
+ * one instruction kind in ctas_per_sm x SMs CTAs of `threads` threads and writes h_out[4] HOST
+ * float64: [0] warp-instructions (Philox test: warp-calls) per clock per scheduler, from the
+ * slowest CTA's clock64 span; [1] that span in SM clocks; [2] kernel milliseconds (CUDA events);
+ * [3] thread-steps (Philox test: calls) per second over the whole GPU.  Synchronises. */
+int  pcmd_pipe_bench(int32_t test, int32_t ctas_per_sm, int32_t threads, int32_t iters, double *h_out);
+const char *pcmd_pipe_bench_name(int32_t test);
+
 #ifdef __cplusplus
 }
 #endif

@@ -12,7 +12,7 @@ import re
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-_LIB_PATH = os.path.join(_HERE, "libpcmd.so")
+_LIB_PATH = os.environ.get("PCMD_LIBRARY") or os.path.join(_HERE, "libpcmd.so")   # PCMD_LIBRARY: an alternative build
 _HEADER = os.path.join(os.path.dirname(_HERE), "include", "pcmd.h")
 
 LIKE_POISSON, LIKE_GAUSS, LIKE_GAUSS_LITERAL = 0, 1, 2
@@ -87,6 +87,9 @@ def lib():
         L.pcmd_debug_philox.argtypes = [u64, vp, i64, vp]
         L.pcmd_status.argtypes = [vp, vp]
         L.pcmd_last_cuda_error.argtypes = [vp]
+        L.pcmd_pipe_bench.argtypes = [i32, i32, i32, i32, vp]
+        L.pcmd_pipe_bench_name.argtypes = [i32]
+        L.pcmd_pipe_bench_name.restype = C.c_char_p
         L.pcmd_launch_count.argtypes = [vp]
         L.pcmd_launch_count.restype = i64
         L.pcmd_profile.argtypes = [vp, i32]
@@ -108,6 +111,23 @@ def _np(a):
 
 def _dp(t):
     return None if t is None else t.data_ptr()
+
+
+def pipe_bench(ctas_per_sm: int = 2, threads: int = 512, iters: int = 4096):
+    """pcmd_pipe_bench for every test: list of dicts {name, rate, cycles, ms, steps_per_s}."""
+    out = []
+    t = 0
+    while True:
+        name = lib().pcmd_pipe_bench_name(t)
+        if name is None:
+            return out
+        r = np.zeros(4)
+        rc = lib().pcmd_pipe_bench(t, ctas_per_sm, threads, iters, _np(r))
+        if rc:
+            raise PcmdError(rc, "pcmd_pipe_bench")
+        out.append(dict(name=name.decode(), rate=float(r[0]), cycles=float(r[1]), ms=float(r[2]),
+                        steps_per_s=float(r[3])))
+        t += 1
 
 
 def philox(seed: int, ctr) -> np.ndarray:

@@ -11,7 +11,7 @@ import sys
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
-LIB = os.path.join(HERE, "libpcmd.so")
+LIB = os.environ.get("PCMD_LIBRARY") or os.path.join(HERE, "libpcmd.so")   # PCMD_LIBRARY: an alternative build
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-shared"]
 
@@ -29,7 +29,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
     stale = (not os.path.exists(LIB)) or any(os.path.getmtime(s) > os.path.getmtime(LIB) for s in _deps())
     if force or stale:
         nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-        cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-o", LIB] + sources()
+        extra = os.environ.get("PCMD_NVCC_EXTRA", "").split()      # e.g. -DS2_PX=1 (tuning experiments)
+        cmd = [nvcc] + NVCC_FLAGS + extra + (["-Xptxas", "-v"] if verbose else []) + ["-o", LIB] + sources()
         subprocess.run(cmd, check=True)
     return LIB
 

@@ -479,7 +479,6 @@ __global__ void __launch_bounds__(S2_THREADS, S2_MINB) k_stage2(const S2Args a) 
     uint32_t pix[S2_PX];
     PhiloxPix ph[S2_PX];                 // the group-independent part of the Philox rounds, per pixel
     uint32_t mctr = 0;
-    int since_flush = 0;
     // stage and phase parity of chunk q and of chunk q-1 (kept as counters: no division in the loop)
     int s = 0, sp = 0;
     uint32_t par = 0, parp = 0;
@@ -501,7 +500,6 @@ __global__ void __launch_bounds__(S2_THREADS, S2_MINB) k_stage2(const S2Args a) 
                 ph[i] = philox_pix_setup(a.key0, a.key1, pix[i], mctr);
             }
             st.reset();
-            since_flush = 0;
         }
         const PointRec *rec = a.rec + (size_t)mt * a.Jpad;
         const uint32_t *tab = a.tab + (size_t)mt * a.cap;
@@ -509,15 +507,24 @@ __global__ void __launch_bounds__(S2_THREADS, S2_MINB) k_stage2(const S2Args a) 
         const uint32_t xs = smem_u32(stab + (size_t)s * S2_TABW);
         const float cx = -(float)(xs >> 2);
         const int ng = d.ng;
+#ifndef S2_UNROLL
+#define S2_UNROLL 1
+#endif
+#define S2_PRAGMA_(x) _Pragma(#x)
+#define S2_PRAGMA_UNROLL(n) S2_PRAGMA_(unroll n)
 #define S2_LOOP(BODY)                                                                          \
-        for (int g = 0; g < ng; ++g) {                                                         \
-            const GroupRec *gr = sb + g;                                                       \
-            uint32_t u[S2_PX][4];                                                              \
-            const PhiloxGrp pq = philox_grp_setup(a.key0, mctr, gr->g_orig);                   \
-            _Pragma("unroll") for (int i = 0; i < S2_PX; ++i)                                  \
-                philox_stage2(a.key0, a.key1, ph[i], pq, u[i]);                                \
-            BODY;                                                                              \
-            if ((g & (S2_FLUSH - 1)) == S2_FLUSH - 1) st.flush();                              \
+        for (int g0 = 0; g0 < ng; g0 += S2_FLUSH) {     /* fp32 sums of at most S2_FLUSH groups, then into fp64 */ \
+            const int g1 = min(ng, g0 + S2_FLUSH);                                             \
+            S2_PRAGMA_UNROLL(S2_UNROLL)                                                        \
+            for (int g = g0; g < g1; ++g) {                                                    \
+                const GroupRec *gr = sb + g;                                                   \
+                uint32_t u[S2_PX][4];                                                          \
+                const PhiloxGrp pq = philox_grp_setup(a.key0, mctr, gr->g_orig);               \
+                _Pragma("unroll") for (int i = 0; i < S2_PX; ++i)                              \
+                    philox_stage2(a.key0, a.key1, ph[i], pq, u[i]);                            \
+                BODY;                                                                          \
+            }                                                                                  \
+            st.flush();                                                                        \
         }
         if (d.cls == S2_CLS_L0) { S2_LOOP((group_rare<NB, COUNTS>(st, gr, u, rec, tab, a.mult))) }
         else if (d.cls == S2_CLS_L1) { S2_LOOP((group_short<NB, COUNTS, 1>(st, gr, u, rec, tab, a.mult))) }
@@ -532,8 +539,6 @@ __global__ void __launch_bounds__(S2_THREADS, S2_MINB) k_stage2(const S2Args a) 
         // every warp has normally left long ago, so nobody waits for the slowest warp
         __syncwarp();
         if (lane == 0) mbar_arrive(&sh.empty[s]);
-        since_flush = ng >= S2_FLUSH ? (ng & (S2_FLUSH - 1)) : since_flush + ng;   // groups since the last flush
-        if (since_flush >= S2_FLUSH || (d.flags & S2_F_LAST)) { st.flush(); since_flush = 0; }
         if (d.flags & S2_F_LAST) {
             // partial flux of this unit; exact integer counts by atomics (parity build)
 #pragma unroll
