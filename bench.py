@@ -327,40 +327,82 @@ def run_ours(args):
 
 
 def run_hbm_stages(args):
-    """HBM fraction of stages 4-5 and 6 on an L2-exceeding batch: the images of
-    `--hbm-batch` models of config `--config` geometry (default c4: 256x256 px, 2 bands) exceed the L2
-    several times, so every stage streams from / to HBM.  Prints one JSON line."""
+    """HBM fraction of stage 4 alone (noise off), the fused stages 4-5 and stage 6 on an L2-exceeding batch
+    (DESIGN.md "Rooflines"): the images of `--hbm-batch` models of config `--config` geometry (default c4:
+    256x256 px, 2 bands) exceed the L2 several times, so every stage streams from / to HBM.  Also: the general
+    2-D K x K convolution against the FP32 FMA peak, and stage 6 on a collapsed pCMD
+    (every pixel in a handful of bins: the shared-memory atomic contention case).
+    Prints one JSON line."""
     import torch
     import paper_1904_00011_b200 as G
     torch.cuda.set_device(0)
-    wl = W.config(args.config)
-    g = G.Pcmd(wl, separable=True)
     n = args.hbm_batch
-    prm = batch_params(wl, n)
-    mag = torch.empty((n, g.B, g.N, g.N), dtype=torch.float32, device="cuda")
-    H = torch.empty((n, g.bins_total), dtype=torch.int32, device="cuda")
-    g.profile(True)
-    acc = np.zeros(5)
     reps = max(args.steps, 3)
-    for it in range(2 + reps):
-        g.simulate(prm, seed=1, mag=mag)
-        g.hess(mag, out=H)
-        ms = g.stage_ms()
-        if it >= 2:
-            acc += np.maximum(ms, 0.0)
-    acc /= reps
     peaks, which = measured_peaks()
-    img_bytes = n * g.B * g.P * 4
-    used = len({b for h in g.hess_specs for b in (h["band_plus"], h["band_minus"], h["band_y"])})
-    s45 = 2 * img_bytes / (acc[2] * 1e-3) / 1e9
-    s6 = (n * len(g.hess_specs) * 0 + n * used * g.P * 4 + n * g.bins_total * 4) / (acc[3] * 1e-3) / 1e9
-    print(json.dumps({"hbm_stages": {
-        "workload": "c%d geometry x %d models (%.0f MB of images, L2 126 MB)" % (args.config, n, img_bytes / 1e6),
-        "stage4_5": {"ms": float(acc[2]), "algorithmic_bytes": 2 * img_bytes, "GBps": s45, "frac": s45 / peaks["hbm_gbs"]},
-        "stage6": {"ms": float(acc[3]), "algorithmic_bytes": n * used * g.P * 4 + n * g.bins_total * 4, "GBps": s6,
-                   "frac": s6 / peaks["hbm_gbs"]},
-        "stage2_ms": float(acc[1]), "peak_GBps": peaks["hbm_gbs"], "peak_source": which}}), flush=True)
-    g.close()
+
+    def timed(wl, separable, n_models, collapsed=False):
+        g = G.Pcmd(wl, separable=separable)
+        prm = batch_params(wl, n_models)
+        mag = torch.empty((n_models, g.B, g.N, g.N), dtype=torch.float32, device="cuda")
+        H = torch.empty((n_models, g.bins_total), dtype=torch.int32, device="cuda")
+        g.profile(True)
+        acc = np.zeros(5)
+        for it in range(2 + reps):
+            g.simulate(prm, seed=1, mag=mag)
+            if collapsed and it == 0:      # every pixel of every image within +-0.01 mag of one point inside the window
+                h0 = g.hess_specs[0]
+                yc = 0.5 * (h0["y_lo"] + h0["y_hi"]); xc = 0.5 * (h0["x_lo"] + h0["x_hi"])
+                base = torch.rand((n_models, 1, g.N, g.N), device="cuda") * 0.02 - 0.01
+                cmag = torch.empty_like(mag)
+                for b in range(g.B):
+                    cmag[:, b:b + 1] = yc + base + (xc if b == h0["band_plus"] and b != h0["band_minus"] else 0.0)
+            g.hess(cmag if collapsed else mag, out=H)
+            ms = g.stage_ms()
+            if it >= 2:
+                acc += np.maximum(ms, 0.0)
+        acc /= reps
+        img_bytes = n_models * g.B * g.P * 4
+        used = len({b for h in g.hess_specs for b in (h["band_plus"], h["band_minus"], h["band_y"])})
+        hess_bytes = n_models * used * g.P * 4 + n_models * g.bins_total * 4
+        out = dict(ms45=float(acc[2]), ms6=float(acc[3]), img_bytes=img_bytes, hess_bytes=hess_bytes, K=int(wl["psf_k"]),
+                   pixel_bands=n_models * g.B * g.P, stage2_ms=float(acc[1]))
+        g.close()
+        return out
+
+    def gbs(nbytes, ms):
+        return nbytes / (ms * 1e-3) / 1e9
+
+    wl_on = W.config(args.config)
+    wl_off = dict(wl_on, shot_noise=0, poisson_sky=0, read_sigma=np.zeros(int(wl_on["n_bands"])),
+                  sky=np.zeros(int(wl_on["n_bands"])))
+    if args.hbm_variant != "all":      # one variant only (profiling): stage times on stderr
+        r = timed(wl_on if args.hbm_variant == "on" else wl_off, args.hbm_variant != "general", n,
+                  collapsed=args.hbm_variant == "collapsed")
+        print(json.dumps({"hbm_variant": args.hbm_variant, **r}), flush=True)
+        return
+    on = timed(wl_on, True, n)
+    off = timed(wl_off, True, n)
+    col = timed(wl_off, True, n, collapsed=True)
+    n2 = max(1, n // 8)                    # the K x K kernel is FMA-bound: a smaller batch keeps the run short
+    gen = timed(wl_off, False, n2)
+    fma_peak = SM_COUNT * 128 * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12          # TFLOP/s: 128 FP32 FMA lanes per SM
+    gen_tflops = 2.0 * gen["K"] ** 2 * gen["pixel_bands"] / (gen["ms45"] * 1e-3) / 1e12
+    res = {"hbm_stages": {
+        "workload": "c%d geometry x %d models (%.0f MB of images, L2 126 MB)" % (args.config, n, on["img_bytes"] / 1e6),
+        "stage4_noise_off": {"kernel": "k_conv2<%d> (separable)" % off["K"], "ms": off["ms45"], "algorithmic_bytes": 2 * off["img_bytes"],
+                             "GBps": gbs(2 * off["img_bytes"], off["ms45"]), "frac": gbs(2 * off["img_bytes"], off["ms45"]) / peaks["hbm_gbs"]},
+        "stage4_5": {"kernel": "k_conv2<%d> (separable) + noise + magnitudes" % on["K"], "ms": on["ms45"], "algorithmic_bytes": 2 * on["img_bytes"],
+                     "GBps": gbs(2 * on["img_bytes"], on["ms45"]), "frac": gbs(2 * on["img_bytes"], on["ms45"]) / peaks["hbm_gbs"],
+                     "bound": "alu (one Philox4x32-10 call + Box-Muller + log2 per pixel-band; DESIGN.md)"},
+        "stage4_general_2d": {"kernel": "k_conv_noise (direct K x K)", "models": n2, "ms": gen["ms45"], "flops": 2.0 * gen["K"] ** 2 * gen["pixel_bands"],
+                              "TFLOPs": gen_tflops, "peak_TFLOPs": fma_peak, "frac_of_fp32_fma_peak": gen_tflops / fma_peak},
+        "stage6": {"ms": on["ms6"], "algorithmic_bytes": on["hess_bytes"], "GBps": gbs(on["hess_bytes"], on["ms6"]),
+                   "frac": gbs(on["hess_bytes"], on["ms6"]) / peaks["hbm_gbs"]},
+        "stage6_collapsed": {"ms": col["ms6"], "algorithmic_bytes": col["hess_bytes"], "GBps": gbs(col["hess_bytes"], col["ms6"]),
+                             "frac": gbs(col["hess_bytes"], col["ms6"]) / peaks["hbm_gbs"],
+                             "what": "every pixel within 0.01 mag of one point of the window (PAPER.md:198)"},
+        "peak_GBps": peaks["hbm_gbs"], "peak_source": which}}
+    print(json.dumps(res), flush=True)
 
 
 def run_pipes(args):
@@ -390,6 +432,8 @@ def main():
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--hbm-batch", type=int, default=0,
                     help="instead of the benchmark: HBM fraction of stages 4-6 on this many models (L2-exceeding)")
+    ap.add_argument("--hbm-variant", default="all", choices=["all", "on", "off", "collapsed", "general"],
+                    help="with --hbm-batch: run one variant only (noise on / off, collapsed Hess, general 2-D PSF)")
     ap.add_argument("--pipes", action="store_true",
                     help="instead of the benchmark: instruction-pipe micro-benchmarks (pcmd_pipe_bench), one JSON line")
     args = ap.parse_args()

@@ -161,7 +161,12 @@ extern "C" int pcmd_create(pcmd_ctx **out, const pcmd_config *cfg) {
         rc = upload(c, &c->d_psf, p2, (size_t)B * G2 * K * K);
         free(p2);
         if (rc) { pcmd_destroy(c); return rc; }
-        if (cfg->psf_separable) TRY(upload(c, &c->d_psf_sep, cfg->psf, (size_t)B * 2 * K));
+        if (cfg->psf_separable) {
+            TRY(upload(c, &c->d_psf_sep, cfg->psf, (size_t)B * 2 * K));
+            c->h_psf_sep = (float *)malloc((size_t)B * 2 * K * sizeof(float));
+            if (!c->h_psf_sep) { pcmd_destroy(c); return PCMD_ENOMEM; }
+            memcpy(c->h_psf_sep, cfg->psf, (size_t)B * 2 * K * sizeof(float));
+        }
     }
     {
         uint64_t *mult = (uint64_t *)malloc((size_t)c->Jpad * sizeof(uint64_t));
@@ -192,6 +197,7 @@ extern "C" int pcmd_create(pcmd_ctx **out, const pcmd_config *cfg) {
     TRY(pcmd_build_sky_tables(c));
     TRY(pcmd_build_lfact(c));
     TRY(pcmd_stage2_occupancy(c));
+    TRY(pcmd_conv_setup(c));
 #undef TRY
     cudaDeviceSynchronize();
     *out = c;
@@ -210,7 +216,7 @@ extern "C" void pcmd_destroy(pcmd_ctx *c) {
     if (c->h_pin) cudaFreeHost(c->h_pin);
     if (c->stage_ev_valid) { cudaEventDestroy(c->stage_ev[0]); cudaEventDestroy(c->stage_ev[1]); }
     if (c->prof_made) for (int i = 0; i < 8; ++i) cudaEventDestroy(c->prof_ev[i]);
-    free(c->h_imf_w);
+    free(c->h_imf_w); free(c->h_psf_sep);
     delete c;
 }
 

@@ -175,6 +175,282 @@ __device__ __forceinline__ void noise_mag_epilogue(const CvArgs &a, const float 
     }
 }
 
+
+// ---------------------------------------------------------------------------------------------
+// Separable PSF, register-blocked.  One launch per band, so the 2K PSF factors
+// are kernel parameters with static indices: every FMA of the two passes takes its weight from the
+// constant bank (no register, no shared-memory read).  A CTA makes a 64 x 64 output tile:
+//   load   the halo tile (rows y0-r .. y0+63+r, columns rounded out to multiples of four) with 16-byte
+//          loads, circular wrap applied per 16-byte segment (R-Q9);
+//   rows   each thread makes 4 consecutive outputs of one halo-tile row from a sliding window of K+3
+//          inputs held in registers (16-byte shared-memory loads), 16-byte store of the row result;
+//   cols   each thread makes a 4 (x) x 4 (y) block of outputs from K+3 16-byte loads of row results;
+//   out    stage 5 (noise, magnitude) on the 16 outputs in registers, 16-byte stores.
+// K(4+K+3)/4... per output: 2K FMAs, ~2.4 shared-memory loads and ~0.3 stores (K = 15).
+#define C2_TW 64
+#define C2_TH 64
+#define C2_THREADS 256
+#define C2_KMAX 21
+
+struct Cv2Args {
+    const float *F;      // [n_models][B][P] dusty flux
+    float *mag;          // [n_models][B][P]
+    float *tap_conv;     // optional
+    const uint32_t *sky_tab;
+    PointRec sky_rec;    // this band's Poisson-sky table
+    int N, B, band;
+    int64_t P;
+    int shot_noise, poisson_sky;
+    uint32_t key0, key1, model0;
+    double zp, sky, read_sigma;
+    float fr[C2_KMAX], fc[C2_KMAX];    // row factor, column factor of this band
+};
+
+__device__ __forceinline__ int wrap_any(int v, int N) {
+    v %= N;
+    return v < 0 ? v + N : v;
+}
+
+// zp - 2.5 log10(arg) for arg > 0: exponent by the add-magic-constant trick (no int->float conversion),
+// mantissa by the special-function unit, finished in one fp64 FMA
+__device__ __forceinline__ float mag_of(float arg, double zp) {
+    const uint32_t bits = __float_as_uint(arg);
+    const float e = __uint_as_float(0x4B000000u | (bits >> 23)) - 8388735.0f;      // (2^23 + biased exponent) - 2^23 - 127
+    const float mant = __uint_as_float((bits & 0x007FFFFFu) | 0x3F800000u);
+    return (float)fma((double)(e + __log2f(mant)), -0.75257498915995298, zp);
+}
+__device__ __forceinline__ float sqrt_approx(float x) {
+    float r;
+    asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));     // relative error ~1e-7: moves a magnitude by < 1e-8
+    return r;
+}
+// #{i < 2^D : u > T[i]} in a table padded with 0xFFFFFFFF to 2^D entries (branch-free)
+__device__ __forceinline__ uint32_t count_below_padded(const uint32_t *__restrict__ T, int D, uint32_t u) {
+    uint32_t pos = 0;
+    for (int sft = D - 1; sft >= 0; --sft) {
+        const uint32_t probe = pos + (1u << sft);
+        if (u > T[probe - 1]) pos = probe;
+    }
+    return pos;
+}
+
+// stage 5 for one pixel (R-Q11); `stab`: this band's sky table padded to 2^sky_d entries (shared memory), or the
+// compact table in global memory (sky_d < 0)
+__device__ __forceinline__ float noise_mag_one(const Cv2Args &a, float Gi, uint32_t p, uint32_t mctr, float skyf, float rs2,
+                                               bool psky, bool need_g, const uint32_t *__restrict__ stab, int sky_d) {
+    uint32_t w[4];
+    float g = 0.f;
+    if (need_g) {
+        philox4x32_10(a.key0, a.key1, p, (uint32_t)a.band, mctr, 2u, w);
+        g = normal_f32(w[0], w[1]);
+    }
+    float arg;      // C' - sky
+    if (psky) {
+        philox4x32_10(a.key0, a.key1, p, (uint32_t)a.band, mctr, 3u, w);
+        const uint32_t n = sky_d >= 0 ? count_below_padded(stab, sky_d, w[0]) : count_below(stab, a.sky_rec.len, w[0]);
+        const float Kc = (float)(a.sky_rec.k0 + n);
+        const float var = (a.shot_noise ? fmaxf(Gi, 0.f) : 0.f) + rs2;
+        arg = Gi + (Kc - skyf) + sqrt_approx(var) * g;
+    } else {
+        const float var = (a.shot_noise ? fmaxf(Gi + skyf, 0.f) : 0.f) + rs2;
+        arg = Gi + sqrt_approx(var) * g;
+    }
+    return (arg > 0.f) ? mag_of(arg, a.zp) : __int_as_float(0x7fc00000);
+}
+
+template <int K, bool VEC>
+__global__ void __launch_bounds__(C2_THREADS, 4) k_conv2(const Cv2Args a) {
+    constexpr int R = (K - 1) / 2, RA = (R + 3) & ~3, OFF = RA - R;
+    constexpr int SW = C2_TW + 2 * RA;            // halo-tile row stride (floats), a multiple of 4
+    constexpr int SH = C2_TH + K - 1;             // halo-tile rows
+    constexpr int NV = (OFF + K + 3 + 3) / 4;     // 16-byte loads of one row-pass window
+    constexpr int SKY_CAP = 1024;                 // Poisson-sky thresholds kept in shared memory
+    extern __shared__ __align__(16) float sm[];
+    float *tile = sm;                             // [SH][SW]
+    float *hrow = sm + SH * SW;                   // [SH][C2_TW]
+    uint32_t *ssky = reinterpret_cast<uint32_t *>(hrow + SH * C2_TW);   // [SKY_CAP]
+    const int N = a.N, m = blockIdx.z, mb = m * a.B + a.band, tid = threadIdx.x;
+    const float *F = a.F + (size_t)mb * a.P;
+    const int x0 = blockIdx.x * C2_TW, y0 = blockIdx.y * C2_TH;
+    const bool psky = a.poisson_sky && a.sky > 0.0;
+    int sky_d = -1;                                // log2 of the padded sky table in shared memory; -1: table stays in global memory
+    if (psky && a.sky_rec.len < SKY_CAP) {
+        sky_d = 32 - __clz(a.sky_rec.len);         // 2^sky_d > len: at least one 0xFFFFFFFF pad entry
+        for (int t = tid; t < (1 << sky_d); t += C2_THREADS)
+            ssky[t] = t < (int)a.sky_rec.len ? a.sky_tab[a.sky_rec.off + t] : 0xFFFFFFFFu;
+    }
+    // ---- load: rows y0-R .., columns x0-RA ..; rows past the last needed output row are skipped
+    const int rows_used = min(SH, N - y0 + K - 1);          // halo rows that feed an output row < N
+    // one conditional add / subtract wraps an index when the image is at least as large as the halo tile
+    const bool big = N >= SW && N >= SH;
+    if (VEC) {
+        constexpr int NQ = SW / 4;                 // 16-byte segments per halo row (18 ... 22): one lane each
+        const int lane = tid & 31, wrp = tid >> 5;
+        if (lane < NQ) {
+            int gx = x0 - RA + 4 * lane;           // N % 4 == 0: a segment never straddles the edge
+            if (big) { gx += gx < 0 ? N : 0; gx -= gx >= N ? N : 0; } else gx = wrap_any(gx, N);
+            int gy = y0 - R + wrp;
+            if (big) gy += gy < 0 ? N : 0; else gy = wrap_any(gy, N);
+            const float *src = F + gx;
+            uint32_t dst = (uint32_t)__cvta_generic_to_shared(reinterpret_cast<float4 *>(tile) + wrp * NQ + lane);
+#pragma unroll
+            for (int it = 0; it < (SH + C2_THREADS / 32 - 1) / (C2_THREADS / 32); ++it) {      // all copies in flight at once
+                if (wrp + it * (C2_THREADS / 32) < rows_used) {
+                    if (big) gy -= gy >= N ? N : 0; else gy = wrap_any(gy, N);
+                    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src + (size_t)gy * N) : "memory");
+                    gy += C2_THREADS / 32; dst += (C2_THREADS / 32) * NQ * 16;
+                }
+            }
+        }
+        asm volatile("cp.async.wait_all;" ::: "memory");
+    } else {
+        for (int t = tid; t < rows_used * SW; t += C2_THREADS) {
+            const int i = t / SW, j = t - i * SW;
+            tile[i * SW + j] = F[(size_t)wrap_any(y0 - R + i, N) * N + wrap_any(x0 - RA + j, N)];
+        }
+    }
+    __syncthreads();
+    // ---- row pass: h[i][x] = sum_k fr[k] F[i][x - (k - R)]
+    constexpr int ROW_IT = (SH * (C2_TW / 4) + C2_THREADS - 1) / C2_THREADS;
+#pragma unroll
+    for (int it = 0; it < ROW_IT; ++it) {
+        const int t = tid + it * C2_THREADS;
+        const int i = t / (C2_TW / 4), sgm = t - i * (C2_TW / 4);
+        if (i >= rows_used) break;
+        float v[NV * 4];
+#pragma unroll
+        for (int q = 0; q < NV; ++q) {
+            const float4 f4 = reinterpret_cast<const float4 *>(tile + i * SW)[sgm + q];
+            v[4 * q] = f4.x; v[4 * q + 1] = f4.y; v[4 * q + 2] = f4.z; v[4 * q + 3] = f4.w;
+        }
+        float h[4] = {0.f, 0.f, 0.f, 0.f};
+#pragma unroll
+        for (int k = 0; k < K; ++k)
+#pragma unroll
+            for (int c = 0; c < 4; ++c) h[c] = fmaf(a.fr[k], v[OFF + c + (K - 1) - k], h[c]);
+        reinterpret_cast<float4 *>(hrow + i * C2_TW)[sgm] = make_float4(h[0], h[1], h[2], h[3]);
+    }
+    __syncthreads();
+    // ---- column pass: G[y][x] = sum_k fc[k] h[y - (k - R)][x], 4 x 4 outputs per thread
+    const int xg = tid & 15, yb = tid >> 4;
+    float acc[4][4];
+#pragma unroll
+    for (int j = 0; j < 4; ++j)
+#pragma unroll
+        for (int c = 0; c < 4; ++c) acc[j][c] = 0.f;
+    if (y0 + 4 * yb < N) {
+#pragma unroll
+        for (int n = 0; n < K + 3; ++n) {
+            const float4 hv = reinterpret_cast<const float4 *>(hrow + (4 * yb + n) * C2_TW)[xg];
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                const int k = j + (K - 1) - n;
+                if (k >= 0 && k < K) {
+                    acc[j][0] = fmaf(a.fc[k], hv.x, acc[j][0]); acc[j][1] = fmaf(a.fc[k], hv.y, acc[j][1]);
+                    acc[j][2] = fmaf(a.fc[k], hv.z, acc[j][2]); acc[j][3] = fmaf(a.fc[k], hv.w, acc[j][3]);
+                }
+            }
+        }
+    }
+    // ---- stage 5 on the 16 outputs
+    const uint32_t mctr = a.model0 + (uint32_t)m;
+    const float skyf = (float)a.sky, rs2 = (float)(a.read_sigma * a.read_sigma);
+    const bool need_g = a.shot_noise || a.read_sigma > 0.0;
+    const uint32_t *stab = sky_d >= 0 ? ssky : a.sky_tab + a.sky_rec.off;
+    const int x = x0 + 4 * xg, yt = y0 + 4 * yb;
+    if (x >= N || yt >= N) return;
+    const uint32_t p0 = (uint32_t)yt * (uint32_t)N + (uint32_t)x;
+    float *mag = a.mag + (size_t)mb * a.P + p0;
+    if (VEC && yt + 3 < N) {                        // the whole 4 x 4 block is inside the image, 16-byte stores
+        if (a.tap_conv) {
+#pragma unroll
+            for (int j = 0; j < 4; ++j)
+                *reinterpret_cast<float4 *>(a.tap_conv + (size_t)mb * a.P + p0 + (size_t)j * N) = make_float4(acc[j][0], acc[j][1], acc[j][2], acc[j][3]);
+        }
+        if (!need_g && !psky) {
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                float mg[4];
+#pragma unroll
+                for (int c = 0; c < 4; ++c) mg[c] = (acc[j][c] > 0.f) ? mag_of(acc[j][c], a.zp) : __int_as_float(0x7fc00000);
+                *reinterpret_cast<float4 *>(mag + (size_t)j * N) = make_float4(mg[0], mg[1], mg[2], mg[3]);
+            }
+        } else {
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                float mg[4];
+#pragma unroll
+                for (int c = 0; c < 4; ++c)
+                    mg[c] = noise_mag_one(a, acc[j][c], p0 + (uint32_t)(j * N + c), mctr, skyf, rs2, psky, need_g, stab, sky_d);
+                *reinterpret_cast<float4 *>(mag + (size_t)j * N) = make_float4(mg[0], mg[1], mg[2], mg[3]);
+            }
+        }
+        return;
+    }
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+        if (yt + j >= N) continue;
+#pragma unroll
+        for (int c = 0; c < 4; ++c)
+            if (x + c < N) {
+                const size_t o = (size_t)j * N + c;
+                if (a.tap_conv) a.tap_conv[(size_t)mb * a.P + p0 + o] = acc[j][c];
+                mag[o] = noise_mag_one(a, acc[j][c], p0 + (uint32_t)o, mctr, skyf, rs2, psky, need_g, stab, sky_d);
+            }
+    }
+}
+
+template <int K>
+static size_t conv2_smem() {
+    constexpr int R = (K - 1) / 2, RA = (R + 3) & ~3;
+    return ((size_t)(C2_TH + K - 1) * (C2_TW + 2 * RA) + (size_t)(C2_TH + K - 1) * C2_TW + 1024) * sizeof(float);
+}
+
+template <int K>
+static cudaError_t conv2_launch(const Cv2Args &a, int n_models, cudaStream_t s) {
+    const dim3 grid((a.N + C2_TW - 1) / C2_TW, (a.N + C2_TH - 1) / C2_TH, n_models);
+    const bool vec = (a.N & 3) == 0 && ((reinterpret_cast<uintptr_t>(a.F) | reinterpret_cast<uintptr_t>(a.mag) |
+                                         reinterpret_cast<uintptr_t>(a.tap_conv)) & 15) == 0;
+    if (vec) k_conv2<K, true><<<grid, C2_THREADS, conv2_smem<K>(), s>>>(a);
+    else k_conv2<K, false><<<grid, C2_THREADS, conv2_smem<K>(), s>>>(a);
+    return cudaGetLastError();
+}
+
+// opt-in to > 48 KB of dynamic shared memory (once per ctx, i.e. per device)
+int pcmd_conv_setup(pcmd_ctx *c) {
+#define C2_OPT(K)                                                                                                    \
+    PCMD_CUDA(c, cudaFuncSetAttribute(k_conv2<K, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)conv2_smem<K>())); \
+    PCMD_CUDA(c, cudaFuncSetAttribute(k_conv2<K, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)conv2_smem<K>()));
+    C2_OPT(5) C2_OPT(7) C2_OPT(15) C2_OPT(21)
+#undef C2_OPT
+    return PCMD_OK;
+}
+
+static int launch_conv2(pcmd_ctx *c, int n_models, uint64_t seed, uint32_t model0, float *d_mag, const float *h_fac,
+                        cudaStream_t s) {
+    for (int b = 0; b < c->B; ++b) {
+        Cv2Args a;
+        a.F = c->d_fdust; a.mag = d_mag; a.tap_conv = c->tap_conv; a.sky_tab = c->d_sky_tab; a.sky_rec = c->sky_rec[b];
+        a.N = c->N; a.B = c->B; a.band = b; a.P = c->P; a.shot_noise = c->shot_noise; a.poisson_sky = c->poisson_sky;
+        a.key0 = (uint32_t)(seed & 0xFFFFFFFFull); a.key1 = (uint32_t)(seed >> 32); a.model0 = model0;
+        a.zp = c->zp[b]; a.sky = c->sky[b]; a.read_sigma = c->read_sigma[b];
+        for (int k = 0; k < C2_KMAX; ++k) {
+            a.fr[k] = k < c->K ? h_fac[((size_t)b * 2) * c->K + k] : 0.f;
+            a.fc[k] = k < c->K ? h_fac[((size_t)b * 2 + 1) * c->K + k] : 0.f;
+        }
+        cudaError_t e;
+        switch (c->K) {
+            case 5: e = conv2_launch<5>(a, n_models, s); break;
+            case 7: e = conv2_launch<7>(a, n_models, s); break;
+            case 15: e = conv2_launch<15>(a, n_models, s); break;
+            default: e = conv2_launch<21>(a, n_models, s); break;
+        }
+        c->launches++;
+        if (e != cudaSuccess) { c->last_cuda = (int)e; return PCMD_ECUDA; }
+    }
+    return PCMD_OK;
+}
+
 int pcmd_launch_conv_noise(pcmd_ctx *c, int n_models, uint64_t seed, uint32_t model0, float *d_mag,
                            cudaStream_t s) {
     CvArgs a;
@@ -189,6 +465,8 @@ int pcmd_launch_conv_noise(pcmd_ctx *c, int n_models, uint64_t seed, uint32_t mo
     a.key0 = (uint32_t)(seed & 0xFFFFFFFFull); a.key1 = (uint32_t)(seed >> 32); a.model0 = model0;
     const int K = c->K;
     dim3 grid((c->N + CV_TX - 1) / CV_TX, (c->N + CV_TY - 1) / CV_TY, n_models * c->B);
+    if (c->psf_sep && c->h_psf_sep && (K == 5 || K == 7 || K == 15 || K == 21))
+        return launch_conv2(c, n_models, seed, model0, d_mag, c->h_psf_sep, s);
     if (c->psf_sep) {
         size_t smem = ((size_t)(CV_TX + K - 1) * (CV_TY + K - 1) + (size_t)(CV_TY + K - 1) * CV_TX + 2 * (size_t)K) * sizeof(float);
         const dim3 blk(CV_TX, CV_ROWS);

@@ -87,6 +87,7 @@ struct pcmd_ctx {
     double *d_imf_w, *d_absmag, *d_feh_grid;
     float *d_psf;          // [B][K][K] (a separable PSF expanded)
     float *d_psf_sep;      // [B][2][K] row and column factors of a separable PSF, else NULL
+    float *h_psf_sep;      // host copy of the same (kernel parameters of k_conv2)
     uint64_t *d_mult;      // [Jpad] splitmix64(j)|1
     double *d_lfact;       // ln(d!) table of the Poisson lnL
     DevHess *d_hess_spec;  // [n_hess]
@@ -274,6 +275,7 @@ int pcmd_launch_stage2(pcmd_ctx *c, int n_models, uint64_t seed, uint32_t model0
 int pcmd_stage2_segments(const pcmd_ctx *c, int n_models);
 int pcmd_stage2_tiles(const pcmd_ctx *c);
 int pcmd_stage2_occupancy(pcmd_ctx *c);
+int pcmd_conv_setup(pcmd_ctx *c);
 int pcmd_launch_conv_noise(pcmd_ctx *c, int n_models, uint64_t seed, uint32_t model0, float *d_mag,
                            cudaStream_t s);
 int pcmd_launch_hess(pcmd_ctx *c, const float *d_mag, int n_models, uint32_t *d_hess,
