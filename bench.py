@@ -44,9 +44,9 @@ from workloads import synthetic as W  # noqa: E402
 METRIC = "pcmd_model_evals_per_s"
 UNIT = "evals/s"
 SM_COUNT, SCHED_PER_SM, LANES = 148, 4, 32
-# measured on this pool's B200 (profiles/README.md): a kernel that does nothing but Philox4x32-10
-# delivers 5.13e11 calls/s = 2.05e12 draws/s (the IMAD.WIDE pipe is the tightest pipe of stage 2)
-PHILOX_CEILING_DRAWS = 2.05e12
+# The Philox-only ceiling (a kernel that does nothing but Philox4x32-10 calls) is measured live by
+# pcmd_pipe_bench in every run (outside the timed region): roofline.frac_of_philox_ceiling.
+PHILOX_TEST = "Philox4x32-10 call"
 # dram__bytes_read.sum + dram__bytes_write.sum of one k_stage2 launch from the committed `ncu --set full`
 # capture (profiles/r1d_c3_launches_and_stage2.md); only known for the configuration that was profiled
 NCU_TRAFFIC_BYTES = {("c3", 1): 1.32e6 + 2.62e6}
@@ -160,7 +160,8 @@ def run_reference(args):
     val = 1.0 / per_eval
     sample = "config c%d tables at %dx%d px (%.4g of the pixels), all 7 stages, scaled by pixel count" % (
         args.config, S, S, frac)
-    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
+    line = {"impl": "reference", "extrapolated": bool(frac < 1.0), "sample_n_im": int(S), "scale_factor": 1.0 / frac,
+            "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": per_eval * 1e3,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
             "data": "synthetic", "gpu_launches": 0,
@@ -269,6 +270,9 @@ def run_ours(args):
     ms = np.array([a.elapsed_time(b) for a, b in ev])
     total_ms = max_over_ranks(float(ms.sum()), "cuda")
     g.profile(False)
+    philox_draws = None
+    if rank == 0:       # the Philox-only kernel of the library, same device, same clocks (5 ms)
+        philox_draws = 4.0 * G.pipe_bench(only=PHILOX_TEST)[0]["steps_per_s"]
 
     # ---- end to end through the host-buffer entry point
     for _ in range(2):
@@ -308,7 +312,8 @@ def run_ours(args):
                 "roofline": {"kernel": "k_stage2 (Poisson draws -> pixel flux)", "bound": "alu",
                              "achieved": ach, "peak": peak_inst, "unit": "Tinst/s",
                              "frac": ach / peak_inst, "traffic": NCU_TRAFFIC_BYTES.get(("c%d" % args.config, n)),
-                             "frac_of_philox_ceiling": (draws / (s2_ms * 1e-3)) / PHILOX_CEILING_DRAWS if s2_ms > 0 else None,
+                             "frac_of_philox_ceiling": (draws / (s2_ms * 1e-3)) / philox_draws if s2_ms > 0 else None,
+                             "philox_only_draws_per_s": philox_draws,
                              "i_alg_thread_inst_per_draw": ia, "draws_per_launch": draws,
                              "ms_per_launch": s2_ms, "peak_source": which + " sm_max_mhz"}}
         if world == 1 and not args.no_cpu:
@@ -428,7 +433,10 @@ def main():
     ap.add_argument("--batch", type=int, default=1)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--cpu-sample", type=int, default=256, help="image side of the cpu_baseline sample")
-    ap.add_argument("--ref-sample", type=int, default=128, help="image side of the --impl reference sample")
+    ap.add_argument("--ref-sample", type=int, default=512,
+                    help="image side of the --impl reference sample (default: the full image up to 512 px, i.e. c1-c4 are "
+                         "timed at full size and only c5 is a sample scaled by pixel count; the line says which)")
+    ap.add_argument("--all-configs", action="store_true", help="one line per BASELINE configuration c1 ... c5 (c4 with --batch 64)")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--hbm-batch", type=int, default=0,
                     help="instead of the benchmark: HBM fraction of stages 4-6 on this many models (L2-exceeding)")
@@ -443,6 +451,11 @@ def main():
         run_hbm_stages(args)
     elif args.impl == "reference":
         run_reference(args)
+    elif args.all_configs:
+        for c in (1, 2, 3, 4, 5):
+            a = argparse.Namespace(**vars(args))
+            a.config, a.batch = c, (64 if c == 4 else 1)
+            run_ours(a)
     else:
         run_ours(args)
 

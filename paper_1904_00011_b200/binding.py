@@ -113,14 +113,17 @@ def _dp(t):
     return None if t is None else t.data_ptr()
 
 
-def pipe_bench(ctas_per_sm: int = 2, threads: int = 512, iters: int = 4096):
-    """pcmd_pipe_bench for every test: list of dicts {name, rate, cycles, ms, steps_per_s}."""
+def pipe_bench(ctas_per_sm: int = 2, threads: int = 512, iters: int = 4096, only: str | None = None):
+    """pcmd_pipe_bench for every test (or the one named `only`): list of dicts {name, rate, cycles, ms, steps_per_s}."""
     out = []
     t = 0
     while True:
         name = lib().pcmd_pipe_bench_name(t)
         if name is None:
             return out
+        if only is not None and name.decode() != only:
+            t += 1
+            continue
         r = np.zeros(4)
         rc = lib().pcmd_pipe_bench(t, ctas_per_sm, threads, iters, _np(r))
         if rc:
