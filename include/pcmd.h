@@ -179,6 +179,18 @@ int  pcmd_stage_ms(pcmd_ctx *ctx, float *h_ms);
 int64_t pcmd_launch_count(const pcmd_ctx *ctx);
 const char *pcmd_strerror(int code);
 
+/* HOST-only convenience: the paper's free parameters (Table 1) -> the linear fields of
+ * pcmd_params.  log10_sfh[n_age]: log10 of the stars per pixel formed in each age bin (model S5; the
+ * parametric models S1-S4 are spread over the age grid by the caller, paper_1904_00011_b200/sfh.py);
+ * feh, sigma_feh: mean and width of the Gaussian MDF (M2/M3); log10_ebv: log10 of the median extinction
+ * parameter, sigma_dust its dimensionless log-normal width (E1-E3; E1 = width 0); dmod: distance modulus
+ * (D1/D2).  Writes sfh_out[n_age] (caller's storage, which out->sfh then points to) with libm pow.  Both
+ * the library and any reference implementation consume this OUTPUT, so no transcendental sits between
+ * the caller's numbers and the expected star counts.  Returns PCMD_EINVAL on NULL / non-finite input. */
+int  pcmd_params_from_paper(int32_t n_age, const double *log10_sfh, double feh, double sigma_feh,
+                            double log10_ebv, double sigma_dust, double dmod, double *sfh_out,
+                            pcmd_params *out);
+
 /* Instruction-pipe micro-benchmarks on the current device (measurement support for the stage-2
  * roofline of DESIGN.md "Rooflines"; nothing of the method runs here).  Test `test` (0 <=
  * test < n, pcmd_pipe_bench_name(test) != NULL) runs `iters` iterations of an unrolled stream of

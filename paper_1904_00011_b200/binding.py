@@ -87,6 +87,8 @@ def lib():
         L.pcmd_debug_philox.argtypes = [u64, vp, i64, vp]
         L.pcmd_status.argtypes = [vp, vp]
         L.pcmd_last_cuda_error.argtypes = [vp]
+        L.pcmd_params_from_paper.argtypes = [i32, vp, C.c_double, C.c_double, C.c_double, C.c_double, C.c_double,
+                                             vp, C.POINTER(Params)]
         L.pcmd_pipe_bench.argtypes = [i32, i32, i32, i32, vp]
         L.pcmd_pipe_bench_name.argtypes = [i32]
         L.pcmd_pipe_bench_name.restype = C.c_char_p
@@ -111,6 +113,19 @@ def _np(a):
 
 def _dp(t):
     return None if t is None else t.data_ptr()
+
+
+def params_from_paper(log10_sfh, feh, sigma_feh, log10_ebv, sigma_dust, dmod) -> dict:
+    """pcmd_params_from_paper (Table 1 free parameters -> linear fields): a params dict as the workloads use."""
+    ls = np.ascontiguousarray(log10_sfh, dtype=np.float64)
+    sfh = np.zeros_like(ls)
+    out = Params()
+    rc = lib().pcmd_params_from_paper(ls.size, _np(ls), float(feh), float(sigma_feh), float(log10_ebv),
+                                      float(sigma_dust), float(dmod), _np(sfh), C.byref(out))
+    if rc:
+        raise PcmdError(rc, "pcmd_params_from_paper")
+    return dict(sfh=sfh, feh_mean=out.feh_mean, feh_sigma=out.feh_sigma, dmod=out.dmod,
+                dust_med=out.dust_med, dust_sigma=out.dust_sigma)
 
 
 def pipe_bench(ctas_per_sm: int = 2, threads: int = 512, iters: int = 4096, only: str | None = None):

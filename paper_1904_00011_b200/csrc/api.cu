@@ -483,6 +483,23 @@ extern "C" int pcmd_debug_philox(uint64_t seed, const uint32_t *h_ctr, int64_t n
     return PCMD_OK;
 }
 
+extern "C" int pcmd_params_from_paper(int32_t n_age, const double *log10_sfh, double feh, double sigma_feh,
+                                      double log10_ebv, double sigma_dust, double dmod, double *sfh_out,
+                                      pcmd_params *out) {
+    if (n_age < 1 || !log10_sfh || !sfh_out || !out) return PCMD_EINVAL;
+    if (!isfinite(feh) || !(sigma_feh > 0.0) || !isfinite(sigma_feh) || !isfinite(log10_ebv) ||
+        !(sigma_dust >= 0.0) || !isfinite(sigma_dust) || !isfinite(dmod))
+        return PCMD_EINVAL;
+    for (int a = 0; a < n_age; ++a) {
+        if (isnan(log10_sfh[a]) || log10_sfh[a] == INFINITY) return PCMD_EINVAL;
+        sfh_out[a] = pow(10.0, log10_sfh[a]);        // -inf -> 0 stars in that bin
+    }
+    out->sfh = sfh_out;
+    out->feh_mean = feh; out->feh_sigma = sigma_feh; out->dmod = dmod;
+    out->dust_med = pow(10.0, log10_ebv); out->dust_sigma = sigma_dust;
+    return PCMD_OK;
+}
+
 extern "C" int pcmd_status(pcmd_ctx *c, void *cuda_stream) {
     if (!c) return PCMD_EINVAL;
     PCMD_CUDA(c, cudaStreamSynchronize((cudaStream_t)cuda_stream));
