@@ -242,6 +242,69 @@ int orc_stage2(const orc_config *c, const double *lambda, const double *flux,
     return 0;
 }
 
+/* ------------------------------------------------------------------------
+ * Aggregated sampler (PAPER.md:75 footnote 3; DESIGN.md R-A1): the number of stars of a pixel is one
+ * Poisson draw with mean Lambda = sum_j lambda_j, and, given that number, every star is of point j with
+ * probability lambda_j / Lambda (the counts of independent Poisson variables conditioned on their sum are
+ * multinomial).  In integers, so that any implementation draws the same stars:
+ *   Lambda = sum_j lambda_j added in increasing j;   w_j = (uint64)((lambda_j / Lambda) 2^40 + 0.5);
+ *   C_j = sum_{i<j} w_i,  W = C_J;
+ *   N_p: word 0 of Philox counter (pixel, 0, model, 4) through the R-C2 table of Lambda;
+ *   star s < N_p: counter (pixel, 1 + (s >> 1), model, 4), U = word[2(s&1)] 2^32 + word[2(s&1)+1],
+ *   r = floor(U W / 2^64), the star is of the point j with C_j <= r < C_{j+1}.
+ * Returns 0, -1 (Lambda out of range).  weights_out (optional): w_j. */
+int orc_stage2_agg(const orc_config *c, const double *lambda, const double *flux,
+                   uint64_t seed, uint32_t model, const uint32_t *pix, int64_t n_pix,
+                   double *F_raw, uint32_t *total, uint64_t *hash, uint32_t *counts, uint64_t *weights_out) {
+    const int J = c->n_points, B = c->n_bands;
+    double Lambda = 0.0;
+    for (int j = 0; j < J; ++j) Lambda += lambda[j];
+    uint64_t *C = (uint64_t *)malloc((size_t)(J + 1) * sizeof(uint64_t));
+    C[0] = 0;
+    for (int j = 0; j < J; ++j) {
+        uint64_t w = 0;
+        if (Lambda > 0.0) w = (uint64_t)((lambda[j] / Lambda) * 1099511627776.0 + 0.5);
+        if (weights_out) weights_out[j] = w;
+        C[j + 1] = C[j] + w;
+    }
+    const uint64_t W = C[J];
+    uint64_t *T = NULL; int64_t tcap = 0, k_lo = 0, k_hi = 0, n;
+    while ((n = orc_poisson_table(Lambda, T, tcap, &k_lo, &k_hi)) < -1) {
+        tcap = (-n - 1) * 2; T = (uint64_t *)realloc(T, (size_t)tcap * sizeof(uint64_t));
+    }
+    if (n == -1) { free(T); free(C); return -1; }
+    uint64_t *mult = (uint64_t *)malloc((size_t)J * sizeof(uint64_t));
+    for (int j = 0; j < J; ++j) mult[j] = orc_splitmix64((uint64_t)j) | 1ull;
+#pragma omp parallel for schedule(dynamic, 64)
+    for (int64_t i = 0; i < n_pix; ++i) {
+        uint32_t p = pix ? pix[i] : (uint32_t)i;
+        double F[16];
+        for (int b = 0; b < B; ++b) F[b] = 0.0;
+        uint64_t h = 0; uint32_t w[4];
+        if (counts) for (int j = 0; j < J; ++j) counts[(size_t)i * J + j] = 0;
+        stream_words(seed, p, 0u, model, 4u, w);
+        const uint32_t N = (Lambda > 0.0 && W > 0) ? orc_poisson_draw(T, k_lo, k_hi, w[0]) : 0;
+        for (uint32_t s = 0; s < N; ++s) {
+            if ((s & 1) == 0) stream_words(seed, p, 1u + (s >> 1), model, 4u, w);
+            const uint64_t U = ((uint64_t)w[2 * (s & 1)] << 32) | (uint64_t)w[2 * (s & 1) + 1];
+            const uint64_t r = (uint64_t)(((unsigned __int128)U * (unsigned __int128)W) >> 64);
+            int lo = 0, hi = J;                      /* the j with C[j] <= r < C[j+1]: C[lo] <= r < C[hi] throughout */
+            while (hi - lo > 1) {
+                int mid = (lo + hi) / 2;
+                if (C[mid] <= r) lo = mid; else hi = mid;
+            }
+            for (int b = 0; b < B; ++b) F[b] += flux[(size_t)lo * B + b];
+            h += mult[lo];
+            if (counts) counts[(size_t)i * J + lo] += 1;
+        }
+        if (F_raw) for (int b = 0; b < B; ++b) F_raw[(size_t)b * n_pix + i] = F[b];
+        if (total) total[i] = N;
+        if (hash) hash[i] = h;
+    }
+    free(mult); free(T); free(C);
+    return 0;
+}
+
 int orc_stage2_brute(const orc_config *c, const double *lambda, const double *flux,
                      uint64_t seed, uint32_t model, double *F_raw, uint32_t *total) {
     /* materialise every star: a growing list of (pixel, point) records, one per star,

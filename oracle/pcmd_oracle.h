@@ -92,6 +92,12 @@ int orc_stage1(const orc_config *c, const orc_params *p, double *mdfw, double *l
 int orc_stage2(const orc_config *c, const double *lambda, const double *flux,
                uint64_t seed, uint32_t model, const uint32_t *pix, int64_t n_pix,
                double *F_raw, uint32_t *total, uint64_t *hash, uint32_t *counts);
+/* Aggregated sampler (PAPER.md:75 footnote 3; DESIGN.md R-A1): one Poisson draw of the pixel's number of
+ * stars (mean sum_j lambda_j), then each star placed on a point with probability lambda_j / sum, by
+ * inversion of an integer cumulative table.  Same outputs as orc_stage2; weights_out (optional) [J]. */
+int orc_stage2_agg(const orc_config *c, const double *lambda, const double *flux,
+                   uint64_t seed, uint32_t model, const uint32_t *pix, int64_t n_pix,
+                   double *F_raw, uint32_t *total, uint64_t *hash, uint32_t *counts, uint64_t *weights_out);
 /* Brute force: materialises every star of every pixel one at a time (a list of
  * (pixel, point) records built from the same draws), then sums star by star. */
 int orc_stage2_brute(const orc_config *c, const double *lambda, const double *flux,

@@ -85,6 +85,8 @@ def lib():
         L.orc_loglike_gauss.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int64, C.c_int]
         L.orc_stage2.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_uint64, C.c_uint32,
                                  C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+        L.orc_stage2_agg.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_uint64, C.c_uint32,
+                                     C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
         L.orc_stage2_brute.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_uint64, C.c_uint32,
                                        C.c_void_p, C.c_void_p]
         L.orc_stage3.argtypes = [C.c_void_p, C.c_void_p, C.c_uint64, C.c_uint32, C.c_void_p, C.c_void_p, C.c_void_p]
@@ -214,6 +216,26 @@ class Oracle:
             raise ValueError("orc_stage2 failed")
         return (F, total, h, counts) if want_counts else (F, total, h)
 
+    def stage2_agg(self, lam, flux, seed, model=0, pix=None, want_counts=False):
+        """Aggregated sampler (PAPER.md:75 fn. 3; DESIGN.md R-A1).  Returns (F, total, hash, weights[, counts])."""
+        if pix is None:
+            n, pixp = self.P, None
+        else:
+            pix = np.ascontiguousarray(pix, dtype=np.uint32)
+            n, pixp = pix.size, _p(pix)
+        F = np.zeros((self.B, n))
+        total = np.zeros(n, dtype=np.uint32)
+        h = np.zeros(n, dtype=np.uint64)
+        wts = np.zeros(self.J, dtype=np.uint64)
+        counts = np.zeros((n, self.J), dtype=np.uint32) if want_counts else None
+        lam = np.ascontiguousarray(lam, dtype=np.float64)
+        flux = np.ascontiguousarray(flux, dtype=np.float64)
+        rc = lib().orc_stage2_agg(C.byref(self.cfg), _p(lam), _p(flux), C.c_uint64(seed), model, pixp, n,
+                                  _p(F), _p(total), _p(h), _p(counts), _p(wts))
+        if rc:
+            raise ValueError("orc_stage2_agg failed")
+        return (F, total, h, wts, counts) if want_counts else (F, total, h, wts)
+
     def stage2_brute(self, lam, flux, seed, model=0):
         F = np.zeros((self.B, self.P))
         total = np.zeros(self.P, dtype=np.uint32)
@@ -249,7 +271,10 @@ class Oracle:
     def simulate(self, prm, seed, model=0):
         """Stages 1-5.  Returns a dict with every intermediate."""
         mdfw, lam, flux = self.stage1(prm)
-        F_raw, total, h = self.stage2(lam, flux, seed, model)
+        if int(self.wl.get("sampler_mode", 0) or 0) == 1:
+            F_raw, total, h, _ = self.stage2_agg(lam, flux, seed, model)
+        else:
+            F_raw, total, h = self.stage2(lam, flux, seed, model)
         A, F_dust = self.stage3(prm, F_raw, seed, model)
         G = self.stage4(F_dust)
         mag = self.stage5(G, seed, model)
