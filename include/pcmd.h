@@ -84,6 +84,11 @@ typedef struct {
                                    R-Q19): psf is [B][G*G][K][K] (psf_separable must be 0), the image is
                                    divided into G x G cells of ceil(N/G) pixels and an output pixel is
                                    convolved with the PSF of its cell (index gy*G + gx)              */
+    int32_t        sampler_mode;/* 0: one Poisson draw per (pixel, isochrone point) (R-C1/R-C2);
+                                   1: aggregated sampler (PAPER.md:75 footnote 3, DESIGN.md R-A1): the pixel's
+                                   number of stars is one Poisson(N_pix) draw and every star is placed on a
+                                   point with probability lambda_j / N_pix -- O(N_pix) instead of O(J) random
+                                   numbers per pixel, a different random stream (R-C1 stream 4)        */
 } pcmd_config;
 
 /* One model = the paper's free parameters (Table 1). */

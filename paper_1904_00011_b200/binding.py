@@ -50,7 +50,8 @@ class Config(C.Structure):
                 ("psf_separable", C.c_int32), ("sky", C.c_void_p), ("read_sigma", C.c_void_p),
                 ("shot_noise", C.c_int32), ("poisson_sky", C.c_int32), ("like_floor", C.c_double),
                 ("n_hess", C.c_int32), ("hess", C.c_void_p), ("dust_frac", C.c_double),
-                ("dust_mode", C.c_int32), ("mdf_cut", C.c_double), ("psf_grid", C.c_int32)]
+                ("dust_mode", C.c_int32), ("mdf_cut", C.c_double), ("psf_grid", C.c_int32),
+                ("sampler_mode", C.c_int32)]
 
 
 class Params(C.Structure):
@@ -196,7 +197,7 @@ class Pcmd:
                      _np(k["psf"]), K, int(bool(separable)), _np(k["sky"]), _np(k["read_sigma"]),
                      int(wl["shot_noise"]), int(wl["poisson_sky"]), float(wl.get("like_floor", 0.1)),
                      len(self.hess_specs), C.addressof(hs), float(wl["dust_frac"]), int(wl["dust_mode"]),
-                     float(wl["mdf_cut"]), G)
+                     float(wl["mdf_cut"]), G, int(wl.get("sampler_mode", 0) or 0))
         self._ctx = C.c_void_p()
         rc = lib().pcmd_create(C.byref(self._ctx), C.byref(cfg))
         if rc:

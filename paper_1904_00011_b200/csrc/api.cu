@@ -38,6 +38,11 @@ static void free_scratch(pcmd_ctx *c) {
     cudaFree(c->d_tab); cudaFree(c->d_rec); cudaFree(c->d_grp); cudaFree(c->d_plan);
     cudaFree(c->d_gcls); cudaFree(c->d_arena); cudaFree(c->d_gpos);
     c->d_grp = nullptr; c->d_plan = nullptr; c->d_gcls = nullptr; c->d_arena = nullptr; c->d_gpos = nullptr;
+    cudaFree(c->d_agg_lam); cudaFree(c->d_agg_C); cudaFree(c->d_agg_G); cudaFree(c->d_agg_rawcnt); cudaFree(c->d_agg_klo);
+    cudaFree(c->d_agg_stcnt); cudaFree(c->d_agg_tab); cudaFree(c->d_agg_q); cudaFree(c->d_agg_rec);
+    c->d_agg_lam = nullptr; c->d_agg_C = nullptr; c->d_agg_G = nullptr; c->d_agg_rawcnt = nullptr; c->d_agg_klo = nullptr;
+    c->d_agg_stcnt = nullptr; c->d_agg_tab = nullptr; c->d_agg_q = nullptr; c->d_agg_rec = nullptr;
+    c->agg_tcap = 0; c->agg_models = 0;
     if (c->h_stage) cudaFreeHost(c->h_stage);
     c->d_sfh = nullptr; c->d_model = nullptr; c->d_mdfw = nullptr; c->d_lambda = nullptr;
     c->d_rawcnt = nullptr; c->d_klo = nullptr; c->d_q = nullptr; c->d_stcnt = nullptr;
@@ -46,8 +51,9 @@ static void free_scratch(pcmd_ctx *c) {
 }
 
 // Scratch for n_models models whose sampler tables need at most cap_raw raw entries each.
-static int ensure_scratch(pcmd_ctx *c, int n_models, int64_t cap_raw) {
-    if (n_models <= c->cap_models && cap_raw <= c->cap_raw) return PCMD_OK;
+static int ensure_scratch(pcmd_ctx *c, int n_models, int64_t cap_raw, int64_t agg_tcap) {
+    if (n_models <= c->cap_models && cap_raw <= c->cap_raw && (c->sampler_mode != 1 || agg_tcap <= c->agg_tcap)) return PCMD_OK;
+    if (agg_tcap < c->agg_tcap) agg_tcap = c->agg_tcap;
     const int nm = n_models > c->cap_models ? n_models : c->cap_models;
     const int64_t cr = cap_raw > c->cap_raw ? cap_raw : c->cap_raw;
     cudaDeviceSynchronize();
@@ -75,6 +81,19 @@ static int ensure_scratch(pcmd_ctx *c, int n_models, int64_t cap_raw) {
         c->arena_cap = words;
         PCMD_CUDA(c, cudaMalloc(&c->d_arena, (size_t)nm * words * sizeof(uint32_t)));
     }
+    if (c->sampler_mode == 1) {
+        PCMD_CUDA(c, cudaMalloc(&c->d_agg_lam, (size_t)nm * sizeof(double)));
+        PCMD_CUDA(c, cudaMalloc(&c->d_agg_C, (size_t)nm * (J + 1) * sizeof(uint64_t)));
+        PCMD_CUDA(c, cudaMalloc(&c->d_agg_G, (size_t)nm * 4098 * sizeof(uint32_t)));
+        PCMD_CUDA(c, cudaMalloc(&c->d_agg_rawcnt, (size_t)nm * 2 * sizeof(uint32_t)));
+        PCMD_CUDA(c, cudaMalloc(&c->d_agg_stcnt, (size_t)nm * 2 * sizeof(uint32_t)));
+        PCMD_CUDA(c, cudaMalloc(&c->d_agg_klo, (size_t)nm * sizeof(uint32_t)));
+        PCMD_CUDA(c, cudaMalloc(&c->d_agg_q, (size_t)nm * agg_tcap * sizeof(double)));
+        PCMD_CUDA(c, cudaMalloc(&c->d_agg_tab, (size_t)nm * agg_tcap * sizeof(uint32_t)));
+        PCMD_CUDA(c, cudaMalloc(&c->d_agg_rec, (size_t)nm * sizeof(PointRec)));
+        PCMD_CUDA(c, cudaMemset(c->d_agg_rec, 0, (size_t)nm * sizeof(PointRec)));
+        c->agg_tcap = agg_tcap; c->agg_models = nm;
+    }
     c->h_stage_bytes = (size_t)nm * (c->A * sizeof(double) + sizeof(DevModel));
     PCMD_CUDA(c, cudaMallocHost(&c->h_stage, 2 * c->h_stage_bytes));
     c->cap_models = nm; c->cap_raw = cr;
@@ -88,6 +107,7 @@ extern "C" int pcmd_create(pcmd_ctx **out, const pcmd_config *cfg) {
         cfg->n_age < 1 || cfg->n_feh < 1 || cfg->n_points < 1 || cfg->psf_k < 1 || cfg->psf_k > 63 ||
         (cfg->psf_k & 1) == 0 || cfg->n_hess < 0 || cfg->n_hess > PCMD_MAX_HESS ||
         cfg->dust_mode < 0 || cfg->dust_mode > 2 || cfg->psf_grid < 0 || cfg->psf_grid > 8 ||
+        cfg->sampler_mode < 0 || cfg->sampler_mode > 1 ||
         (cfg->psf_grid > 1 && cfg->psf_separable))
         return PCMD_EINVAL;
     if (!cfg->age_idx || !cfg->feh_idx || !cfg->imf_w || !cfg->absmag || !cfg->feh_grid || !cfg->zp ||
@@ -120,6 +140,7 @@ extern "C" int pcmd_create(pcmd_ctx **out, const pcmd_config *cfg) {
     if (!c) return PCMD_ENOMEM;
     memset(c, 0, sizeof(*c));
     c->N = cfg->n_im; c->B = B; c->A = cfg->n_age; c->Z = cfg->n_feh; c->J = J; c->Jpad = (J + 3) & ~3;
+    c->sampler_mode = cfg->sampler_mode;
     c->K = K; c->psf_sep = cfg->psf_separable; c->shot_noise = cfg->shot_noise != 0;
     c->poisson_sky = cfg->poisson_sky != 0; c->n_hess = cfg->n_hess; c->dust_mode = cfg->dust_mode;
     c->P = (int64_t)cfg->n_im * cfg->n_im; c->hess_bins = bins;
@@ -229,17 +250,20 @@ static int stage_params(pcmd_ctx *c, const pcmd_params *params, int n_models, in
     // upper bound of the raw sampler-table size of one model (sizing only, no method arithmetic):
     // lambda_j <= max_a sfh_a * imf_w_j, and a table spans fewer than 20 sqrt(lambda) + 96 counts.
     int64_t cap = 0;
+    double npix_max = 0.0;          // largest N_pix = sum of the SFH (sizes the Poisson(N_pix) table of the aggregated sampler)
     for (int i = 0; i < n_models; ++i) {
         const pcmd_params &p = params[i];
         if (!p.sfh || !(p.feh_sigma > 0.0) || !isfinite(p.feh_mean) || !isfinite(p.feh_sigma) ||
             !isfinite(p.dmod) || !(p.dust_med >= 0.0) || !isfinite(p.dust_med) || !(p.dust_sigma >= 0.0) ||
             !isfinite(p.dust_sigma))
             return PCMD_EINVAL;
-        double smax = 0.0;
+        double smax = 0.0, ssum = 0.0;
         for (int a = 0; a < c->A; ++a) {
             if (!(p.sfh[a] >= 0.0) || !isfinite(p.sfh[a])) return PCMD_EINVAL;
             if (p.sfh[a] > smax) smax = p.sfh[a];
+            ssum += p.sfh[a];
         }
+        if (ssum > npix_max) npix_max = ssum;
         double tot = 0.0;
         if (smax * c->imf_w_max <= PCMD_LAMBDA_MAX) {
             tot = 20.0 * sqrt(smax) * c->imf_sqrt_sum + 96.0 * c->J;   // sum_j 20 sqrt(smax w_j) + 96
@@ -253,9 +277,11 @@ static int stage_params(pcmd_ctx *c, const pcmd_params *params, int n_models, in
         if ((int64_t)tot > cap) cap = (int64_t)tot;
     }
     if (cap > 0xFFFFFFF0ll) return PCMD_ERANGE;
-    int rc = ensure_scratch(c, n_models, cap);
+    if (c->sampler_mode == 1 && npix_max * 1.0001 > PCMD_LAMBDA_MAX) return PCMD_ERANGE;   // R-C2 covers means up to 2^22
+    const int64_t agg_tcap = (int64_t)(20.0 * sqrt(npix_max * 1.0001 + 1.0) + 96.0);
+    int rc = ensure_scratch(c, n_models, c->sampler_mode == 1 ? 16 : cap, agg_tcap);
     if (rc) return rc;
-    c->n_seg = pcmd_stage2_segments(c, n_real);
+    c->n_seg = c->sampler_mode == 1 ? 1 : pcmd_stage2_segments(c, n_real);
     const int64_t need_img = (int64_t)n_real * c->B * c->P;
     if (need_img > c->fdust_elems) {
         cudaDeviceSynchronize();

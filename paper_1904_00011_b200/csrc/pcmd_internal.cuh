@@ -118,6 +118,12 @@ struct pcmd_ctx {
     uint32_t *d_arena; int64_t arena_cap;  // [cap_models][arena_cap] padded search tables of the D classes
     float *d_part;  int64_t part_elems;  // stage-2 partial fluxes [realisations][n_seg][B][P]
     int32_t n_seg, s2_ctas_per_sm;
+    // aggregated sampler (sampler_mode = 1, agg.cu): total lambda, cumulative integer weights, guide cells and the
+    // R-C2 table of the total, per model
+    int32_t sampler_mode;
+    double *d_agg_lam; uint64_t *d_agg_C; uint32_t *d_agg_G;
+    uint32_t *d_agg_rawcnt, *d_agg_klo, *d_agg_stcnt, *d_agg_tab; double *d_agg_q; PointRec *d_agg_rec;
+    int64_t agg_tcap; int32_t agg_models; size_t smem_agg;
     int32_t *d_status;     // device status word
     // hess / loglike scratch
     pcmd_hess_stats *d_hpart; int64_t hpart_cap; // per-block partial stats
@@ -269,6 +275,11 @@ __device__ __forceinline__ uint32_t count_below(const uint32_t *__restrict__ T, 
 // launchers implemented in the stage files ---------------------------------------------------
 int pcmd_launch_stage1(pcmd_ctx *c, int n_models, cudaStream_t s);
 int pcmd_build_sky_tables(pcmd_ctx *c);
+int pcmd_build_tables(pcmd_ctx *c, const double *d_lambda, int J, int n_models, uint32_t *rawcnt, uint32_t *klo,
+                      double *q, int64_t cap, uint32_t *stcnt, uint32_t *tab, PointRec *rec, int Jpad, cudaStream_t s);
+int pcmd_launch_agg_tables(pcmd_ctx *c, int n_models, cudaStream_t s);
+int pcmd_launch_stage2_agg(pcmd_ctx *c, int n_models, uint64_t seed, uint32_t model0, uint64_t *d_hash,
+                           uint32_t *d_total, cudaStream_t s);
 int pcmd_build_lfact(pcmd_ctx *c);
 int pcmd_launch_stage2(pcmd_ctx *c, int n_models, uint64_t seed, uint32_t model0, float *d_flux_raw,
                        uint64_t *d_hash, uint32_t *d_total, cudaStream_t s);

@@ -385,9 +385,9 @@ __global__ void __launch_bounds__(256) k_group_emit(const PointRec *__restrict__
     }
 }
 
-static int build_tables(pcmd_ctx *c, const double *d_lambda, int J, int n_models, uint32_t *rawcnt,
-                        uint32_t *klo, double *q, int64_t cap, uint32_t *stcnt, uint32_t *tab,
-                        PointRec *rec, int Jpad, cudaStream_t s) {
+int pcmd_build_tables(pcmd_ctx *c, const double *d_lambda, int J, int n_models, uint32_t *rawcnt,
+                      uint32_t *klo, double *q, int64_t cap, uint32_t *stcnt, uint32_t *tab,
+                      PointRec *rec, int Jpad, cudaStream_t s) {
     int total = J * n_models, tb = 128, gb = (total + tb - 1) / tb;
     k_table_range<<<gb, tb, 0, s>>>(d_lambda, J, n_models, rawcnt, klo);
     PCMD_LAUNCHED(c);
@@ -408,7 +408,8 @@ int pcmd_launch_stage1(pcmd_ctx *c, int n_models, cudaStream_t s) {
         c->Z, c->J, c->Jpad, c->B, c->mdf_cut, c->zp[0], c->zp[1], c->zp[2], c->zp[3], c->d_mdfw,
         c->d_lambda, c->d_rec, c->d_status);
     PCMD_LAUNCHED(c);
-    int rc = build_tables(c, c->d_lambda, c->J, n_models, c->d_rawcnt, c->d_klo, c->d_q, c->cap_raw,
+    if (c->sampler_mode == 1) return pcmd_launch_agg_tables(c, n_models, s);     // no per-point tables, no work layout
+    int rc = pcmd_build_tables(c, c->d_lambda, c->J, n_models, c->d_rawcnt, c->d_klo, c->d_q, c->cap_raw,
                           c->d_stcnt, c->d_tab, c->d_rec, c->Jpad, s);
     if (rc) return rc;
     const int n_groups = c->Jpad >> 2;
@@ -443,7 +444,7 @@ int pcmd_build_sky_tables(pcmd_ctx *c) {
     PCMD_CUDA(c, cudaMalloc(&c->d_sky_tab, cap * sizeof(uint32_t)));
     PCMD_CUDA(c, cudaMemset(d_rec, 0, 4 * sizeof(PointRec)));
     PCMD_CUDA(c, cudaMemcpy(d_lam, c->sky, B * sizeof(double), cudaMemcpyHostToDevice));
-    int rc = build_tables(c, d_lam, B, 1, d_raw, d_klo, d_q, cap, d_st, c->d_sky_tab, d_rec, 4, 0);
+    int rc = pcmd_build_tables(c, d_lam, B, 1, d_raw, d_klo, d_q, cap, d_st, c->d_sky_tab, d_rec, 4, 0);
     if (rc) return rc;
     PointRec h[4];
     PCMD_CUDA(c, cudaMemcpy(h, d_rec, 4 * sizeof(PointRec), cudaMemcpyDeviceToHost));

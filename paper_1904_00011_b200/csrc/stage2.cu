@@ -588,7 +588,7 @@ __global__ void __launch_bounds__(S2_THREADS, S2_MINB) k_stage2(const S2Args a) 
 struct RdArgs {
     const float *part; const ModelPlan *plan; const DevModel *mdl;
     float *flux_raw, *flux_dust;
-    int B, n_seg, dust_mode, n_models, mts;
+    int B, n_seg, dust_mode, n_models, mts, n_frag;   // n_frag >= 0: partial fluxes per pixel (else from the plan)
     int64_t P;
     uint32_t key0, key1, model0;
     double dust_frac, coef[4];
@@ -599,7 +599,7 @@ __global__ void __launch_bounds__(256) k_reduce_dust(const RdArgs a) {
     if (idx >= a.P * a.n_models) return;
     const int m = (int)(idx / a.P);
     const uint32_t p = (uint32_t)(idx - (int64_t)m * a.P);
-    const int n_frag = s2_model_segments(a.plan[(size_t)m * a.mts], a.n_seg);   // partial fluxes written per pixel
+    const int n_frag = a.n_frag >= 0 ? a.n_frag : s2_model_segments(a.plan[(size_t)m * a.mts], a.n_seg);   // partial fluxes written per pixel
     float A = 0.f; bool behind = true;
     if (a.dust_mode != 0) {       // fp32: the factor needs 1e-5 relative, expf / exp10f give 1e-7
         const DevModel M = a.mdl[m * a.mts];
@@ -661,6 +661,10 @@ int pcmd_launch_stage2(pcmd_ctx *c, int n_models, uint64_t seed, uint32_t model0
         PCMD_CUDA(c, cudaMemsetAsync(d_hash, 0, (size_t)n_models * c->P * sizeof(uint64_t), s));
         PCMD_CUDA(c, cudaMemsetAsync(d_total, 0, (size_t)n_models * c->P * sizeof(uint32_t), s));
     }
+    if (c->sampler_mode == 1) {      // aggregated sampler (agg.cu): one partial flux per pixel
+        int rc = pcmd_launch_stage2_agg(c, n_models, seed, model0, d_hash, d_total, s);
+        if (rc) return rc;
+    } else {
     const int64_t n_units = (int64_t)n_models * a.n_tiles * a.n_seg;
     const int64_t slots = (int64_t)c->sm_count * (d_hash ? 1 : c->s2_ctas_per_sm);
     const int grid = (int)(n_units < slots ? n_units : slots);
@@ -676,8 +680,10 @@ int pcmd_launch_stage2(pcmd_ctx *c, int n_models, uint64_t seed, uint32_t model0
     else e = launch_s2<4>(a, counts, grid, s);
     c->launches++;
     if (e != cudaSuccess) { c->last_cuda = (int)e; return PCMD_ECUDA; }
+    }
 
     RdArgs r;
+    r.n_frag = c->sampler_mode == 1 ? 1 : -1;
     r.part = c->d_part; r.plan = c->d_plan; r.mdl = c->d_model; r.flux_raw = d_flux_raw; r.flux_dust = c->d_fdust;
     r.mts = c->tab_stride; r.B = c->B; r.n_seg = c->n_seg; r.dust_mode = c->dust_mode;
     r.n_models = n_models; r.P = c->P;
