@@ -215,6 +215,8 @@ def run_ours(args):
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
 
     wl = W.config(args.config)
+    if args.sampler_mode == 1:      # aggregated sampler (PAPER.md:75 fn. 3; DESIGN.md R-A1): a different random stream
+        wl = dict(wl, sampler_mode=1)
     g = G.Pcmd(wl, separable=True)
     prm = batch_params(wl, args.batch)
     n = len(prm)
@@ -244,7 +246,10 @@ def run_ours(args):
         raise SystemExit("device status %d" % g.status())
     # draws of one step on this rank: P x #{j: lambda_j > 0}, summed over the batch's models
     # (models with a narrow MDF have whole isochrones cut to lambda = 0: those are not drawn)
-    draws_step = sum(int((g.debug_weights(i)["lam"] > 0).sum()) for i in range(n)) * g.P
+    if args.sampler_mode == 1:      # random numbers that decide a star: one per star (expected N_pix per pixel) + the total
+        draws_step = int(sum(float(np.sum(p["sfh"])) + 1.0 for p in prm) * g.P)
+    else:
+        draws_step = sum(int((g.debug_weights(i)["lam"] > 0).sum()) for i in range(n)) * g.P
     g.profile(True)
 
     # ---- device-timed leg
@@ -292,14 +297,17 @@ def run_ours(args):
         evals = whole_job_rate(n * args.steps, world, total_ms * 1e-3)
         s2_ms = float(stage[1]) / args.steps
         draws = draws_step
-        ia = i_alg(g.B)
+        # aggregated sampler: half a Philox call per star (10 wide multiplies + 10 xors), the 64 x 64 -> high 64
+        # product (4 wide multiplies), guide look-up + ~2 search steps (8), B flux adds
+        ia = i_alg(g.B) if args.sampler_mode == 0 else 32 + g.B
         peak_inst = SM_COUNT * SCHED_PER_SM * LANES * float(peaks.get("sm_max_mhz", 1965.0)) * 1e6 / 1e12
         ach = draws * ia / (s2_ms * 1e-3) / 1e12 if s2_ms > 0 else 0.0
         line = {"metric": METRIC, "value": evals, "unit": UNIT, "n_gpus": world, "steps": args.steps,
                 "warmup": max(args.warmup, 3), "ms_per_step": ms_step, "higher_is_better": True,
                 "scaling": "weak", "vs_baseline": None, "dtype": "u32+f32", "data": "synthetic",
                 "config": {"workload": "c%d" % args.config, "n_im": g.N, "n_bands": g.B, "n_points": g.J,
-                           "batch": n, "psf_k": int(wl["psf_k"]), "l2": "flushed between steps (2x L2 written)",
+                           "batch": n, "psf_k": int(wl["psf_k"]),
+                           "sampler": "aggregated (sampler_mode 1)" if args.sampler_mode == 1 else "per-point Poisson (sampler_mode 0)", "l2": "flushed between steps (2x L2 written)",
                            "parallelism": "replicas over model index x%d" % world},
                 "draws_per_s": draws * world * args.steps / (total_ms * 1e-3),
                 "draws_per_s_stage2": draws / (s2_ms * 1e-3) if s2_ms > 0 else None,
@@ -309,7 +317,7 @@ def run_ours(args):
                 "clocks": clk,
                 "e2e": {"value": n * world * args.steps / e2e_s, "unit": UNIT,
                         "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h)},
-                "roofline": {"kernel": "k_stage2 (Poisson draws -> pixel flux)", "bound": "alu",
+                "roofline": {"kernel": "k_stage2_agg (stars placed by table inversion)" if args.sampler_mode == 1 else "k_stage2 (Poisson draws -> pixel flux)", "bound": "alu",
                              "achieved": ach, "peak": peak_inst, "unit": "Tinst/s",
                              "frac": ach / peak_inst, "traffic": NCU_TRAFFIC_BYTES.get(("c%d" % args.config, n)),
                              "frac_of_philox_ceiling": (draws / (s2_ms * 1e-3)) / philox_draws if s2_ms > 0 else None,
@@ -440,6 +448,8 @@ def main():
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--hbm-batch", type=int, default=0,
                     help="instead of the benchmark: HBM fraction of stages 4-6 on this many models (L2-exceeding)")
+    ap.add_argument("--sampler-mode", type=int, default=0, choices=[0, 1],
+                    help="0: one Poisson draw per (pixel, point), the headline path; 1: aggregated sampler (PAPER.md:75 fn. 3)")
     ap.add_argument("--hbm-variant", default="all", choices=["all", "on", "off", "collapsed", "general"],
                     help="with --hbm-batch: run one variant only (noise on / off, collapsed Hess, general 2-D PSF)")
     ap.add_argument("--pipes", action="store_true",

@@ -8,7 +8,7 @@
 
 #define AGG_SHIFT 28                 // guide cell = r >> 28 (r < W ~ 2^40: 4096 cells, + 2 for W slightly above 2^40)
 #define AGG_CELLS 4098
-#define AGG_THREADS 256
+#define AGG_THREADS 512
 
 // One block per model.  Lambda = sum_j lambda_j in increasing j (thread 0: the order is part of the definition),
 // w_j = (uint64)((lambda_j / Lambda) 2^40 + 0.5), C = exclusive prefix sums (integers: any order), guide cells.
@@ -21,11 +21,27 @@ __global__ void __launch_bounds__(1024) k_agg_tables(const double *__restrict__ 
     const int m = blockIdx.x;
     const double *lam = lambda_all + (size_t)m * J;
     uint64_t *C = C_all + (size_t)m * (J + 1);
-    if (threadIdx.x == 0) {
-        double t = 0.0;
-        for (int j = 0; j < J; ++j) t = __dadd_rn(t, lam[j]);
-        s_tot = t; lam_tot[m] = t; carry = 0ull;
+    // the sum is sequential by definition; thread 0 walks chunks staged in shared memory (coalesced loads by the block)
+    __shared__ double s_chunk[2048];
+    double t = 0.0;
+    for (int base = 0; base < J; base += 2048) {
+        const int n = min(2048, J - base);
+        for (int i = threadIdx.x; i < n; i += blockDim.x) s_chunk[i] = lam[base + i];
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            int i = 0;
+            for (; i + 8 <= n; i += 8) {
+                double v[8];
+#pragma unroll
+                for (int k = 0; k < 8; ++k) v[k] = s_chunk[i + k];
+#pragma unroll
+                for (int k = 0; k < 8; ++k) t = __dadd_rn(t, v[k]);
+            }
+            for (; i < n; ++i) t = __dadd_rn(t, s_chunk[i]);
+        }
+        __syncthreads();
     }
+    if (threadIdx.x == 0) { s_tot = t; lam_tot[m] = t; carry = 0ull; }
     __syncthreads();
     const double tot = s_tot;
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
@@ -111,19 +127,24 @@ __global__ void __launch_bounds__(AGG_THREADS) k_stage2_agg(const AggArgs a) {
     }
     double F[4] = {0.0, 0.0, 0.0, 0.0};
     uint64_t h = 0;
-    for (uint32_t s = 0; s < N; ++s) {
-        if ((s & 1u) == 0u) philox4x32_10(a.key0, a.key1, p, 1u + (s >> 1), mctr, 4u, w);
-        const uint64_t U = (s & 1u) ? (((uint64_t)w[2] << 32) | w[3]) : (((uint64_t)w[0] << 32) | w[1]);
-        const uint64_t r = __umul64hi(U, W);
-        const uint32_t cell = (uint32_t)(r >> AGG_SHIFT);
-        int lo = (int)G[cell], hi = (int)G[cell + 1];
-        while (lo < hi) {                           // the j with C_j <= r < C_{j+1}
-            const int mid = (lo + hi + 1) >> 1;
-            if (C[mid] <= r) lo = mid; else hi = mid - 1;
+    // two stars per Philox call, their two searches interleaved (independent chains)
+    for (uint32_t s = 0; s < N; s += 2) {
+        philox4x32_10(a.key0, a.key1, p, 1u + (s >> 1), mctr, 4u, w);
+        const uint64_t r0 = __umul64hi(((uint64_t)w[0] << 32) | w[1], W), r1 = __umul64hi(((uint64_t)w[2] << 32) | w[3], W);
+        int lo0 = (int)G[(uint32_t)(r0 >> AGG_SHIFT)], hi0 = (int)G[(uint32_t)(r0 >> AGG_SHIFT) + 1];
+        int lo1 = (int)G[(uint32_t)(r1 >> AGG_SHIFT)], hi1 = (int)G[(uint32_t)(r1 >> AGG_SHIFT) + 1];
+        while (lo0 < hi0 || lo1 < hi1) {            // the j with C_j <= r < C_{j+1}
+            const int m0 = (lo0 + hi0 + 1) >> 1, m1 = (lo1 + hi1 + 1) >> 1;
+            const uint64_t c0 = C[m0], c1 = C[m1];
+            if (lo0 < hi0) { if (c0 <= r0) lo0 = m0; else hi0 = m0 - 1; }
+            if (lo1 < hi1) { if (c1 <= r1) lo1 = m1; else hi1 = m1 - 1; }
         }
-        const float4 f = *reinterpret_cast<const float4 *>(rec[lo].f);
-        F[0] += (double)f.x; F[1] += (double)f.y; F[2] += (double)f.z; F[3] += (double)f.w;
-        if (COUNTS) h += a.mult[lo];
+        const bool two = s + 1 < N;
+        const float4 f0 = *reinterpret_cast<const float4 *>(rec[lo0].f);
+        const float4 f1 = two ? *reinterpret_cast<const float4 *>(rec[lo1].f) : make_float4(0.f, 0.f, 0.f, 0.f);
+        F[0] += (double)f0.x; F[1] += (double)f0.y; F[2] += (double)f0.z; F[3] += (double)f0.w;
+        F[0] += (double)f1.x; F[1] += (double)f1.y; F[2] += (double)f1.z; F[3] += (double)f1.w;
+        if (COUNTS) { h += a.mult[lo0]; if (two) h += a.mult[lo1]; }
     }
     for (int b = 0; b < a.B; ++b) a.part[((size_t)m * a.B + b) * a.P + p] = (float)F[b];
     if (COUNTS) { a.total[(size_t)m * a.P + p] = N; a.hash[(size_t)m * a.P + p] = h; }
