@@ -219,6 +219,8 @@ def run_ours(args):
         wl = dict(wl, sampler_mode=1)
     g = G.Pcmd(wl, separable=True)
     prm = batch_params(wl, args.batch)
+    if args.sfh_scale != 1.0:       # diagnostic: the same tables with every expected star count scaled (1e-6: every group of
+        prm = [dict(p, sfh=np.asarray(p["sfh"]) * args.sfh_scale) for p in prm]   # points in the rare-star class = Philox + one vote)
     n = len(prm)
     seed, m0 = int(wl["seed"]), shard_models(n, rank)
     data = np.concatenate([d.ravel() for d in wl["data_hess"]]).astype(np.uint32)
@@ -306,7 +308,7 @@ def run_ours(args):
                 "warmup": max(args.warmup, 3), "ms_per_step": ms_step, "higher_is_better": True,
                 "scaling": "weak", "vs_baseline": None, "dtype": "u32+f32", "data": "synthetic",
                 "config": {"workload": "c%d" % args.config, "n_im": g.N, "n_bands": g.B, "n_points": g.J,
-                           "batch": n, "psf_k": int(wl["psf_k"]),
+                           "batch": n, "psf_k": int(wl["psf_k"]), **({"sfh_scale": args.sfh_scale} if args.sfh_scale != 1.0 else {}),
                            "sampler": "aggregated (sampler_mode 1)" if args.sampler_mode == 1 else "per-point Poisson (sampler_mode 0)", "l2": "flushed between steps (2x L2 written)",
                            "parallelism": "replicas over model index x%d" % world},
                 "draws_per_s": draws * world * args.steps / (total_ms * 1e-3),
@@ -448,6 +450,8 @@ def main():
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--hbm-batch", type=int, default=0,
                     help="instead of the benchmark: HBM fraction of stages 4-6 on this many models (L2-exceeding)")
+    ap.add_argument("--sfh-scale", type=float, default=1.0,
+                    help="diagnostic: multiply every model's SFH (N_pix) by this factor; not a BASELINE workload")
     ap.add_argument("--sampler-mode", type=int, default=0, choices=[0, 1],
                     help="0: one Poisson draw per (pixel, point), the headline path; 1: aggregated sampler (PAPER.md:75 fn. 3)")
     ap.add_argument("--hbm-variant", default="all", choices=["all", "on", "off", "collapsed", "general"],

@@ -20,15 +20,17 @@ struct __align__(16) PointRec {
 // sorted by class; a class is cut into chunks (the unit of shared-memory staging); the chunks of all
 // (model, pixel tile) pairs form one cost-weighted sequence that is cut into equal shares, one per
 // persistent CTA (no work queue, no atomics).
-#define S2_NCLASS 8        // classes, most expensive first:
+#define S2_NCLASS 10       // classes, most expensive first:
 #define S2_CLS_D9 1        //   0 bisection in global memory (tables longer than 511)
 #define S2_CLS_D7 2        //   1-3 branch-free search of a padded table of 2^D words in shared memory
 #define S2_CLS_D5 3
-#define S2_CLS_L4 4        //   4-6 L inline thresholds decide the draw (more stars: probability < 2^-10)
-#define S2_CLS_L2 5
-#define S2_CLS_L1 6
-#define S2_CLS_L0 7        //   7 rare: P(any star) < 2^-8 per draw: one max-compare per group, then class L1's path
-#define S2_CLS_NONE 8      //   no point of the group can have a star: dropped
+#define S2_CLS_S4 4        //   4-5 the same search over the first 2^D - 1 thresholds only (k0 = 0 and more stars than that
+#define S2_CLS_S3 5        //       have probability < 2^-10: the overflow path finishes them)
+#define S2_CLS_L4 6        //   6-8 L inline thresholds decide the draw (more stars: probability < 2^-10)
+#define S2_CLS_L2 7
+#define S2_CLS_L1 8
+#define S2_CLS_L0 9        //   9 rare: P(any star) < 2^-8 per draw: one max-compare per group, then class L1's path
+#define S2_CLS_NONE 10     //   no point of the group can have a star: dropped
 #define S2_CHUNK 48         // group records per staged chunk (48 * 160 B = 7.5 KB)
 #define S2_TABW 4096        // words of staged search tables per chunk (16 KB): 32 / 8 / 2 groups of D5 / D7 / D9
 // cost model of the static partition: ~SM cycles per warp and group of each class loop (profiles/), and per chunk
@@ -36,15 +38,22 @@ struct __align__(16) PointRec {
 #define S2_COST_D9 420u
 #define S2_COST_D7 340u
 #define S2_COST_D5 250u
+#define S2_COST_S4 225u
+#define S2_COST_S3 205u
 #define S2_COST_L4 190u
 #define S2_COST_L2 160u
 #define S2_COST_L1 155u
 #define S2_COST_L0 150u
 #define S2_COST_CHUNK 100u
+// log2 of the padded table size of a search class
+__host__ __device__ __forceinline__ int s2_class_depth(int cls) {
+    return cls == S2_CLS_D9 ? 9 : (cls == S2_CLS_D7 ? 7 : (cls == S2_CLS_D5 ? 5 : (cls == S2_CLS_S4 ? 4 : (cls == S2_CLS_S3 ? 3 : 0))));
+}
 struct __align__(16) GroupRec {      // 160 bytes
     uint32_t g_orig, cls, tmin, pad1; // original group index (Philox counter word 1), class, min over w of T[0][w]
     uint32_t T[5][4];                 // T[i][w]: (i+1)-th stored threshold minus 1 of point w; 0xFFFFFFFF if none.
-                                      // Search classes D5/D7/D9: T[4][w] = float bits of (float)k0
+                                      // Search classes: T[4][w] = float bits of k0 - (table offset in the stage buffer);
+                                      // S3/S4: T[3][w] = the overflow threshold (the 2^D-th stored threshold minus 1)
     float f[4][4];                    // f[w][b]: flux of one star of point w in band b
 };
 // Per model: the class-sorted group list cut into chunks.  Chunk i of class c (chunk_start[c] <= i <

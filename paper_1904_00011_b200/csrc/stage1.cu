@@ -222,6 +222,8 @@ __device__ __forceinline__ int point_class(const PointRec &r, const uint32_t *__
         if (r.len <= 1 || tab[r.off + 1] >= S2_OVF_THR) return S2_CLS_L1;
         if (r.len <= 2 || tab[r.off + 2] >= S2_OVF_THR) return S2_CLS_L2;
         if (r.len <= 4 || tab[r.off + 4] >= S2_OVF_THR) return S2_CLS_L4;
+        if (r.len <= 7 || tab[r.off + 7] >= S2_OVF_THR) return S2_CLS_S3;
+        if (r.len <= 15 || tab[r.off + 15] >= S2_OVF_THR) return S2_CLS_S4;
     }
     if (r.len <= 31) return S2_CLS_D5;
     if (r.len <= 127) return S2_CLS_D7;
@@ -249,7 +251,7 @@ __global__ void __launch_bounds__(256) k_group_classify(const PointRec *__restri
 //
 // Cost model of stage 2 (cost units ~ SM cycles per warp and group, measured per class loop with
 // ncu, profiles/): the static partition of the chunk sequence among the persistent CTAs is by cost.
-__constant__ uint32_t c_s2_group_cost[S2_NCLASS] = {S2_COST_G, S2_COST_D9, S2_COST_D7, S2_COST_D5,
+__constant__ uint32_t c_s2_group_cost[S2_NCLASS] = {S2_COST_G, S2_COST_D9, S2_COST_D7, S2_COST_D5, S2_COST_S4, S2_COST_S3,
                                                     S2_COST_L4, S2_COST_L2, S2_COST_L1, S2_COST_L0};
 __global__ void __launch_bounds__(1024) k_group_sort(const uint8_t *__restrict__ cls_all, int Jpad,
                                                      int64_t arena_cap, uint32_t *__restrict__ pos_all,
@@ -295,12 +297,12 @@ __global__ void __launch_bounds__(1024) k_group_sort(const uint8_t *__restrict__
         ModelPlan t;
         // padded search tables: D9 first, then D7, D5; a class that does not fit the arena is
         // demoted to bisection in global memory (run_cls = 0)
-        const int64_t stride[4] = {0, 4 << 9, 4 << 7, 4 << 5};
+        const int64_t stride[6] = {0, 4 << 9, 4 << 7, 4 << 5, 4 << 4, 4 << 3};      // words of padded tables per group
         int first_d = S2_CLS_D9;
         for (;;) {
             int64_t need = 0;
-            for (int c = first_d; c <= S2_CLS_D5; ++c) need += stride[c] * (int64_t)count[c];
-            if (need <= arena_cap || first_d > S2_CLS_D5) break;
+            for (int c = first_d; c <= S2_CLS_S3; ++c) need += stride[c] * (int64_t)count[c];
+            if (need <= arena_cap || first_d > S2_CLS_S3) break;
             first_d++;
         }
         int64_t off = 0;
@@ -309,11 +311,11 @@ __global__ void __launch_bounds__(1024) k_group_sort(const uint8_t *__restrict__
         for (int c = 0; c < S2_NCLASS; ++c) {
             t.cls_start[c] = (int32_t)cls_start[c];
             t.arena_off[c] = 0;
-            const bool in_arena = c >= first_d && c <= S2_CLS_D5;
+            const bool in_arena = c >= first_d && c <= S2_CLS_S3;
             if (in_arena) { t.arena_off[c] = off; off += stride[c] * (int64_t)count[c]; }
-            const bool demoted = c >= S2_CLS_D9 && c <= S2_CLS_D5 && !in_arena;
+            const bool demoted = c >= S2_CLS_D9 && c <= S2_CLS_S3 && !in_arena;
             t.run_cls[c] = demoted ? 0 : c;
-            const int cg = in_arena ? (int)(S2_TABW / stride[c]) : S2_CHUNK;     // groups per chunk
+            const int cg = in_arena ? min((int)(S2_TABW / stride[c]), S2_CHUNK) : S2_CHUNK;     // groups per chunk
             t.chunk_groups[c] = cg;
             t.chunk_cost[c] = (uint32_t)cg * c_s2_group_cost[t.run_cls[c]] + S2_COST_CHUNK;
             const int n = (int)count[c], nch = (n + cg - 1) / cg;
@@ -358,28 +360,29 @@ __global__ void __launch_bounds__(256) k_group_emit(const PointRec *__restrict__
         if (w == 0) { o->g_orig = (uint32_t)g; o->cls = (uint32_t)cls; o->tmin = tmin; o->pad1 = 0; }
 #pragma unroll
         for (int i = 0; i < 5; ++i) o->T[i][w] = ((uint32_t)i < r.len) ? tab[r.off + i] : 0xFFFFFFFFu;
-        if (cls <= S2_CLS_D5) {
+        if (cls <= S2_CLS_S3) {
             // the search classes keep the first count here: k0 (bisection class), or, for a class whose padded
             // tables are staged in shared memory, the float k0 - (word offset of the point's table in its
             // chunk's stage buffer): stage 2 then gets the count from the ADDRESS of the found entry
             const ModelPlan *pl = plan_all + m;
             if (cls >= pl->first_d) {
-                const int D = cls == S2_CLS_D9 ? 9 : (cls == S2_CLS_D7 ? 7 : 5);
+                const int D = s2_class_depth(cls);
                 const int g_local = ((int)pos - pl->cls_start[cls]) % pl->chunk_groups[cls];
                 o->T[4][w] = __float_as_uint((float)((int)r.k0 - ((g_local * 4 + w) << D)));
+                if (cls >= S2_CLS_S4) o->T[3][w] = ((1u << D) - 1u < r.len) ? tab[r.off + (1u << D) - 1u] : 0xFFFFFFFFu;
             } else o->T[4][w] = r.k0;
         }
 #pragma unroll
         for (int b = 0; b < 4; ++b) o->f[w][b] = r.f[b];
     }
     const ModelPlan *t = plan_all + m;
-    if (cls >= t->first_d && cls <= S2_CLS_D5) {
-        const int D = cls == S2_CLS_D9 ? 9 : (cls == S2_CLS_D7 ? 7 : 5);
+    if (cls >= t->first_d && cls <= S2_CLS_S3) {
+        const int D = s2_class_depth(cls);
         uint32_t *dst = arena_all + (size_t)m * arena_cap + t->arena_off[cls] +
                         (int64_t)((int)pos - t->cls_start[cls]) * (4 << D);
 #pragma unroll
         for (int w = 0; w < 4; ++w) {
-            const uint32_t off = rec[4 * g + w].off, len = rec[4 * g + w].len;
+            const uint32_t off = rec[4 * g + w].off, len = min(rec[4 * g + w].len, (1u << D) - 1u);   // S3/S4: the first 2^D - 1 only
             for (int i = lane; i < (1 << D); i += 32) dst[(w << D) + i] = ((uint32_t)i < len) ? tab[off + i] : 0xFFFFFFFFu;
         }
     }

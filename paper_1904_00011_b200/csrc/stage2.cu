@@ -297,11 +297,15 @@ __device__ __forceinline__ void group_generic(S2State<NB, COUNTS> &st, const Gro
 // FADD (FMA pipe), and the count comes out of the final address with an FMUL and an FMA -- no integer
 // add, no int->float conversion.  xs: byte address of this group's four tables; cx = -(stage buffer
 // address) / 4 as a float; the record holds k0 - (word offset of the table in the stage buffer).
-template <int NB, bool COUNTS, int D>
+template <int NB, bool COUNTS, int D, bool OVF>
 __device__ __forceinline__ void group_search(S2State<NB, COUNTS> &st, const GroupRec *__restrict__ g,
                                              const uint32_t (&u)[S2_PX][4], uint32_t xs, float cx,
+                                             const PointRec *__restrict__ rec, const uint32_t *__restrict__ tab,
                                              const uint64_t *__restrict__ mult) {
     const float4 K = *reinterpret_cast<const float4 *>(g->T[4]);
+    const uint4 TO = *reinterpret_cast<const uint4 *>(g->T[3]);     // classes S3/S4: the overflow thresholds
+    const uint32_t tov[4] = {TO.x, TO.y, TO.z, TO.w};
+    bool ovf = false;
     const float kq[4] = {K.x + cx, K.y + cx, K.z + cx, K.w + cx};                  // k0 - (address of X[0]) / 4
 #pragma unroll
     for (int w = 0; w < 4; ++w) {
@@ -312,6 +316,7 @@ __device__ __forceinline__ void group_search(S2State<NB, COUNTS> &st, const Grou
 #pragma unroll
         for (int i = 0; i < S2_PX; ++i) {
             const uint32_t x = u[i][w];
+            if (OVF) ovf |= x > tov[w];
             float off = (x > t0) ? hi : lo;                                         // bits = byte address of X[pos]
 #pragma unroll
             for (int sft = D - 2; sft >= 0; --sft) {
@@ -322,6 +327,21 @@ __device__ __forceinline__ void group_search(S2State<NB, COUNTS> &st, const Grou
             // off = (address of X[pos]) 2^-149 -> address / 4 + kq = k0 + pos, in two exact steps (2^147 is not a float)
             const float nf = fmaf(off * 8.507059173023462e37f, 2097152.0f, kq[w]);
             add_stars<NB, COUNTS>(st, i, nf, f, g->g_orig * 4u + w, mult);
+        }
+    }
+    // S3/S4: more stars than the 2^D - 1 searched thresholds (probability < 2^-10 per draw): the rest of the table
+    if (OVF && __any_sync(0xffffffffu, ovf)) {
+#pragma unroll
+        for (int w = 0; w < 4; ++w) {
+            const uint32_t j = g->g_orig * 4u + (uint32_t)w;
+#pragma unroll
+            for (int i = 0; i < S2_PX; ++i) {
+                if (u[i][w] > tov[w]) {
+                    const PointRec r = rec[j];
+                    const uint32_t extra = 1u + count_below(tab + r.off + (1u << D), r.len - (1u << D), u[i][w]);
+                    add_stars<NB, COUNTS>(st, i, (float)extra, *reinterpret_cast<const float4 *>(g->f[w]), j, mult);
+                }
+            }
         }
     }
 }
@@ -413,7 +433,7 @@ __device__ __forceinline__ void s2_issue(const S2Args &a, S2Shared &sh, GroupRec
     const int g0 = p.cls_start[cls] + li * cg;
     const int ng = min(cg, p.cls_start[cls + 1] - g0);
     const int run = p.run_cls[cls];
-    const int D = run == S2_CLS_D9 ? 9 : (run == S2_CLS_D7 ? 7 : (run == S2_CLS_D5 ? 5 : 0));
+    const int D = s2_class_depth(run);
     const uint32_t rbytes = (uint32_t)ng * (uint32_t)sizeof(GroupRec), tbytes = D ? ((uint32_t)ng << (D + 4)) : 0u;
     const GroupRec *rsrc = a.grp + (size_t)mt * a.n_groups + g0;
     const uint32_t *tsrc = a.arena + (size_t)mt * a.arena_cap + p.arena_off[cls] + ((size_t)(g0 - p.cls_start[cls]) << (D + 2));
@@ -530,9 +550,11 @@ __global__ void __launch_bounds__(S2_THREADS, S2_MINB) k_stage2(const S2Args a) 
         else if (d.cls == S2_CLS_L1) { S2_LOOP((group_short<NB, COUNTS, 1>(st, gr, u, rec, tab, a.mult))) }
         else if (d.cls == S2_CLS_L2) { S2_LOOP((group_short<NB, COUNTS, 2>(st, gr, u, rec, tab, a.mult))) }
         else if (d.cls == S2_CLS_L4) { S2_LOOP((group_four<NB, COUNTS>(st, gr, u, rec, tab, a.mult))) }
-        else if (d.cls == S2_CLS_D5) { S2_LOOP((group_search<NB, COUNTS, 5>(st, gr, u, xs + ((uint32_t)g << 9), cx, a.mult))) }
-        else if (d.cls == S2_CLS_D7) { S2_LOOP((group_search<NB, COUNTS, 7>(st, gr, u, xs + ((uint32_t)g << 11), cx, a.mult))) }
-        else if (d.cls == S2_CLS_D9) { S2_LOOP((group_search<NB, COUNTS, 9>(st, gr, u, xs + ((uint32_t)g << 13), cx, a.mult))) }
+        else if (d.cls == S2_CLS_S3) { S2_LOOP((group_search<NB, COUNTS, 3, true>(st, gr, u, xs + ((uint32_t)g << 7), cx, rec, tab, a.mult))) }
+        else if (d.cls == S2_CLS_S4) { S2_LOOP((group_search<NB, COUNTS, 4, true>(st, gr, u, xs + ((uint32_t)g << 8), cx, rec, tab, a.mult))) }
+        else if (d.cls == S2_CLS_D5) { S2_LOOP((group_search<NB, COUNTS, 5, false>(st, gr, u, xs + ((uint32_t)g << 9), cx, rec, tab, a.mult))) }
+        else if (d.cls == S2_CLS_D7) { S2_LOOP((group_search<NB, COUNTS, 7, false>(st, gr, u, xs + ((uint32_t)g << 11), cx, rec, tab, a.mult))) }
+        else if (d.cls == S2_CLS_D9) { S2_LOOP((group_search<NB, COUNTS, 9, false>(st, gr, u, xs + ((uint32_t)g << 13), cx, rec, tab, a.mult))) }
         else { S2_LOOP((group_generic<NB, COUNTS>(st, gr, u, rec, tab, a.mult))) }
 #undef S2_LOOP
         // the stage is free once every warp has arrived; warp 0 refills the PREVIOUS chunk's stage, which
