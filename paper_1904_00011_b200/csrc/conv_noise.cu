@@ -465,7 +465,10 @@ int pcmd_launch_conv_noise(pcmd_ctx *c, int n_models, uint64_t seed, uint32_t mo
     a.key0 = (uint32_t)(seed & 0xFFFFFFFFull); a.key1 = (uint32_t)(seed >> 32); a.model0 = model0;
     const int K = c->K;
     dim3 grid((c->N + CV_TX - 1) / CV_TX, (c->N + CV_TY - 1) / CV_TY, n_models * c->B);
-    if (c->psf_sep && c->h_psf_sep && (K == 5 || K == 7 || K == 15 || K == 21))
+    // k_conv2 (64 x 64 tiles, one launch per band) when a launch fills the GPU; small jobs take the 32 x 32-tile kernel
+    // below in one launch over all bands (4x the CTAs: latency-bound there, not bandwidth-bound)
+    const int64_t ctas2 = (int64_t)((c->N + C2_TW - 1) / C2_TW) * ((c->N + C2_TH - 1) / C2_TH) * n_models;
+    if (c->psf_sep && c->h_psf_sep && (K == 5 || K == 7 || K == 15 || K == 21) && ctas2 >= 2 * (int64_t)c->sm_count)
         return launch_conv2(c, n_models, seed, model0, d_mag, c->h_psf_sep, s);
     if (c->psf_sep) {
         size_t smem = ((size_t)(CV_TX + K - 1) * (CV_TY + K - 1) + (size_t)(CV_TY + K - 1) * CV_TX + 2 * (size_t)K) * sizeof(float);

@@ -3,7 +3,9 @@
 // (north_star; R-Q15) and the paper's Eq. 2-4 (R-Q14).
 #include "pcmd_internal.cuh"
 
-#define HS_THREADS 256
+#ifndef HS_THREADS
+#define HS_THREADS 512
+#endif
 #define HS_PIX_PER_BLOCK 4096
 
 // Binning arithmetic, fp32, no contraction:
@@ -130,31 +132,10 @@ __global__ void k_hess_stats(const pcmd_hess_stats *__restrict__ part, int nblk,
 int pcmd_launch_hess(pcmd_ctx *c, const float *d_mag, int n_models, uint32_t *d_hess,
                      pcmd_hess_stats *d_stats, cudaStream_t s) {
     // Pixels per block: at least HS_PIX_PER_BLOCK (a block zeroes and flushes a whole private histogram, so long
-    // pixel runs amortise that).  A batch that fills the GPU by itself takes 1 ... 8 blocks per diagram, whichever
-    // leaves the last wave of CTAs fullest (one block per diagram also saves the memset, the global atomics and
-    // the stats kernel: worth ~15 %).
-    int maxbins0 = 0;
-    for (int h = 0; h < c->n_hess; ++h) maxbins0 = max(maxbins0, c->hess[h].nx * c->hess[h].ny);
-    int per_sm = 0;
-    if ((size_t)maxbins0 * 4 <= 200 * 1024) {
-        if ((size_t)maxbins0 * 4 > 48 * 1024 && (size_t)maxbins0 * 4 > c->smem_hess) {
-            PCMD_CUDA(c, cudaFuncSetAttribute(k_hess<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, maxbins0 * 4));
-            c->smem_hess = (size_t)maxbins0 * 4;
-        }
-        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_hess<true>, HS_THREADS, (size_t)maxbins0 * 4);
-    }
-    if (per_sm < 1) per_sm = 4;
-    const int64_t slots = (int64_t)c->sm_count * per_sm, diagrams = (int64_t)n_models * c->n_hess;
-    int64_t want_blocks = (slots * 2) / diagrams;
-    if (diagrams >= slots / 2) {
-        double best = -1.0;
-        for (int nb = 1; nb <= 8; ++nb) {
-            if (nb > 1 && c->P / nb < HS_PIX_PER_BLOCK) break;
-            const double waves = (double)(diagrams * nb) / (double)slots;
-            const double eff = waves / ceil(waves) * (nb == 1 ? 1.0 : 0.85);
-            if (eff > best + 1e-9) { best = eff; want_blocks = nb; }
-        }
-    }
+    // pixel runs amortise that); a batch that fills the GPU by itself takes one block per diagram, which also
+    // saves the memset, the global atomics and the stats kernel (measured: splitting diagrams to fill the last
+    // wave of CTAs costs more than it gains).
+    int64_t want_blocks = ((int64_t)c->sm_count * 8) / ((int64_t)n_models * c->n_hess);
     if (want_blocks < 1) want_blocks = 1;
     int64_t ppb = (c->P + want_blocks - 1) / want_blocks;
     if (ppb < HS_PIX_PER_BLOCK) ppb = HS_PIX_PER_BLOCK;
