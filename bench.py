@@ -47,9 +47,10 @@ SM_COUNT, SCHED_PER_SM, LANES = 148, 4, 32
 # The Philox-only ceiling (a kernel that does nothing but Philox4x32-10 calls) is measured live by
 # pcmd_pipe_bench in every run (outside the timed region): roofline.frac_of_philox_ceiling.
 PHILOX_TEST = "Philox4x32-10 call"
-# dram__bytes_read.sum + dram__bytes_write.sum of one k_stage2 launch from the committed `ncu --set full`
-# capture (profiles/r1d_c3_launches_and_stage2.md); only known for the configuration that was profiled
-NCU_TRAFFIC_BYTES = {("c3", 1): 1.32e6 + 2.62e6}
+# dram__bytes_read.sum + dram__bytes_write.sum of one k_stage2 launch from the committed captures: c3 and c5 from
+# `ncu --set full` (profiles/r2_stage2.md), c4 x 64 models from the `--metrics` launch list (profiles/r2_launches.md);
+# None for configurations / batches that were not captured
+NCU_TRAFFIC_BYTES = {("c3", 1): 1.323e6 + 0.195e6, ("c5", 1): 12.376e6 + 0.042e6, ("c4", 64): 40.84e6 + 2.91e6}
 
 
 def i_alg(n_bands: int) -> int:
