@@ -36,7 +36,7 @@ static void free_scratch(pcmd_ctx *c) {
     cudaFree(c->d_sfh); cudaFree(c->d_model); cudaFree(c->d_mdfw); cudaFree(c->d_lambda);
     cudaFree(c->d_rawcnt); cudaFree(c->d_klo); cudaFree(c->d_q); cudaFree(c->d_stcnt);
     cudaFree(c->d_tab); cudaFree(c->d_rec); cudaFree(c->d_grp); cudaFree(c->d_plan);
-    cudaFree(c->d_gcls); cudaFree(c->d_arena); cudaFree(c->d_gpos);
+    cudaFree(c->d_gcls); cudaFree(c->d_arena); cudaFree(c->d_gpos); cudaFree(c->d_alloc); c->d_alloc = nullptr;
     c->d_grp = nullptr; c->d_plan = nullptr; c->d_gcls = nullptr; c->d_arena = nullptr; c->d_gpos = nullptr;
     cudaFree(c->d_agg_lam); cudaFree(c->d_agg_C); cudaFree(c->d_agg_G); cudaFree(c->d_agg_rawcnt); cudaFree(c->d_agg_klo);
     cudaFree(c->d_agg_stcnt); cudaFree(c->d_agg_tab); cudaFree(c->d_agg_q); cudaFree(c->d_agg_rec);
@@ -66,6 +66,7 @@ static int ensure_scratch(pcmd_ctx *c, int n_models, int64_t cap_raw, int64_t ag
     PCMD_CUDA(c, cudaMalloc(&c->d_rawcnt, (size_t)nm * (J + 1) * sizeof(uint32_t)));
     PCMD_CUDA(c, cudaMalloc(&c->d_stcnt, (size_t)nm * (J + 1) * sizeof(uint32_t)));
     PCMD_CUDA(c, cudaMalloc(&c->d_klo, (size_t)nm * J * sizeof(uint32_t)));
+    PCMD_CUDA(c, cudaMalloc(&c->d_alloc, (size_t)nm * 2 * sizeof(uint32_t)));
     PCMD_CUDA(c, cudaMalloc(&c->d_q, (size_t)nm * cr * sizeof(double)));
     PCMD_CUDA(c, cudaMalloc(&c->d_tab, (size_t)nm * cr * sizeof(uint32_t)));
     PCMD_CUDA(c, cudaMalloc(&c->d_rec, (size_t)nm * Jp * sizeof(PointRec)));
@@ -462,19 +463,21 @@ extern "C" int pcmd_debug_weights(pcmd_ctx *c, int32_t model, double *h_lambda, 
         if (h_k0) h_k0[j] = rec[j].k0;
         if (h_len) h_len[j] = rec[j].len;
         if (h_flux) for (int b = 0; b < c->B; ++b) h_flux[(size_t)j * c->B + b] = rec[j].f[b];
-        total += rec[j].len;   // tables are compact and in point order
+        total += rec[j].len;
     }
-    free(rec);
     if (n_tables) *n_tables = total;
-    if (h_tables) {
-        int64_t n = total < cap ? total : cap;
-        uint32_t *tmp = (uint32_t *)malloc((size_t)(n ? n : 1) * sizeof(uint32_t));
-        if (!tmp) return PCMD_ENOMEM;
-        e = cudaMemcpy(tmp, c->d_tab + (size_t)model * c->cap_raw, (size_t)n * sizeof(uint32_t), cudaMemcpyDeviceToHost);
-        if (e != cudaSuccess) { free(tmp); c->last_cuda = (int)e; return PCMD_ECUDA; }
-        for (int64_t i = 0; i < n; ++i) h_tables[i] = tmp[i] + 1u;  // stored minus 1 on the device
+    if (h_tables && c->sampler_mode != 1) {
+        // tables are compact but placed in completion order (k_points): gathered here in point order
+        uint32_t *tmp = (uint32_t *)malloc((size_t)(c->cap_raw ? c->cap_raw : 1) * sizeof(uint32_t));
+        if (!tmp) { free(rec); return PCMD_ENOMEM; }
+        e = cudaMemcpy(tmp, c->d_tab + (size_t)model * c->cap_raw, (size_t)c->cap_raw * sizeof(uint32_t), cudaMemcpyDeviceToHost);
+        if (e != cudaSuccess) { free(tmp); free(rec); c->last_cuda = (int)e; return PCMD_ECUDA; }
+        int64_t o = 0;
+        for (int j = 0; j < J && o < cap; ++j)
+            for (uint32_t i = 0; i < rec[j].len && o < cap; ++i) h_tables[o++] = tmp[rec[j].off + i] + 1u;  // stored minus 1 on the device
         free(tmp);
     }
+    free(rec);
     return PCMD_OK;
 }
 

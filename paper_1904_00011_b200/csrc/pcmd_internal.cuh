@@ -32,7 +32,9 @@ struct __align__(16) PointRec {
 #define S2_CLS_L0 9        //   9 rare: P(any star) < 2^-8 per draw: one max-compare per group, then class L1's path
 #define S2_CLS_NONE 10     //   no point of the group can have a star: dropped
 #define S2_CHUNK 48         // group records per staged chunk (48 * 160 B = 7.5 KB)
+#ifndef S2_TABW
 #define S2_TABW 4096        // words of staged search tables per chunk (16 KB): 32 / 8 / 2 groups of D5 / D7 / D9
+#endif
 // cost model of the static partition: ~SM cycles per warp and group of each class loop (profiles/), and per chunk
 #define S2_COST_G 1500u
 #define S2_COST_D9 420u
@@ -113,6 +115,7 @@ struct pcmd_ctx {
     double *d_mdfw;        // [cap_models][Z]
     double *d_lambda;      // [cap_models][J]
     uint32_t *d_rawcnt;    // [cap_models][J+1] raw table range sizes -> exclusive offsets
+    uint32_t *d_alloc;     // [cap_models][2] bump allocators of the raw and the compact table regions (k_points)
     uint32_t *d_klo;       // [cap_models][J]
     double *d_q;           // [cap_models][cap_raw] pmf ratios, then thresholds (as uint64)
     uint32_t *d_stcnt;     // [cap_models][J+1] stored counts -> exclusive offsets

@@ -333,6 +333,114 @@ __global__ void __launch_bounds__(1024) k_group_sort(const uint8_t *__restrict__
     }
 }
 
+// Stage 1 for one point per thread, fused (the main path; the separate kernels above still build the few
+// tables of the Poisson sky and of the aggregated sampler): MDF weights (thread 0 of the block, R-C3 order),
+// lambda_j, per-star fluxes, the R-C2 table (range pass, raw entries into a scratch region taken from a
+// per-model bump allocator, thresholds, compaction into a second bump-allocated region), the point record
+// and the class of the point's group.  Table regions are handed out in completion order, so their PLACE
+// varies from run to run; their contents, and everything stage 2 computes from them, do not.
+__global__ void __launch_bounds__(128) k_points(const DevModel *__restrict__ mdl, const double *__restrict__ sfh,
+                         const double *__restrict__ feh_grid, const int32_t *__restrict__ age_idx,
+                         const int32_t *__restrict__ feh_idx, const double *__restrict__ imf_w,
+                         const double *__restrict__ absmag, int A, int Z, int J, int Jpad, int B,
+                         double mdf_cut, double zp0, double zp1, double zp2, double zp3,
+                         double *__restrict__ mdfw_out, double *__restrict__ lambda_out,
+                         double *__restrict__ qbuf, int64_t cap, uint32_t *__restrict__ tab_all,
+                         uint32_t *__restrict__ alloc, PointRec *__restrict__ rec_out,
+                         uint8_t *__restrict__ gcls_out, int32_t *status) {
+    extern __shared__ double w[];  // [Z]
+    const int m = blockIdx.y;
+    const DevModel M = mdl[m];
+    if (threadIdx.x == 0) {
+        double e_min = INFINITY;
+        for (int z = 0; z < Z; ++z) {
+            double d = __dsub_rn(feh_grid[z], M.feh_mean);
+            w[z] = __ddiv_rn(__dmul_rn(d, d), __dmul_rn(__dmul_rn(2.0, M.feh_sigma), M.feh_sigma));
+            if (w[z] < e_min) e_min = w[z];
+        }
+        double G = 0.0;
+        for (int z = 0; z < Z; ++z) { w[z] = expneg_basic(__dsub_rn(w[z], e_min)); G = __dadd_rn(G, w[z]); }
+        double G2 = 0.0;
+        for (int z = 0; z < Z; ++z) {
+            w[z] = __ddiv_rn(w[z], G);
+            if (w[z] < mdf_cut) w[z] = 0.0;
+            G2 = __dadd_rn(G2, w[z]);
+        }
+        for (int z = 0; z < Z; ++z) {
+            w[z] = __ddiv_rn(w[z], G2);
+            if (blockIdx.x == 0) mdfw_out[(size_t)m * Z + z] = w[z];
+        }
+    }
+    __syncthreads();
+    const double zp[4] = {zp0, zp1, zp2, zp3};
+    const int j = blockIdx.x * blockDim.x + threadIdx.x;
+    PointRec r;
+    r.T0 = 0xFFFFFFFFu; r.off = 0; r.len = 0; r.k0 = 0;
+    r.f[0] = r.f[1] = r.f[2] = r.f[3] = 0.f;
+    int pcls = S2_CLS_NONE;
+    if (j < J) {
+        const double lam = __dmul_rn(__dmul_rn(sfh[(size_t)m * A + age_idx[j]], w[feh_idx[j]]), imf_w[j]);
+        lambda_out[(size_t)m * J + j] = lam;
+        if (!(lam >= 0.0) || lam > PCMD_LAMBDA_MAX) atomicMin(status, PCMD_ERANGE);
+        for (int b = 0; b < B; ++b)  // fluxes according to the distance
+            r.f[b] = (float)exp10(-0.4 * (absmag[(size_t)j * B + b] + M.dmod - zp[b]));
+        if (lam > 0.0 && lam <= PCMD_LAMBDA_MAX) {
+            // R-C2 step 1: range of the relative pmf >= 2^-64
+            const long long mode = (long long)floor(lam);
+            long long k_hi = mode, k_lo = mode;
+            double v = 1.0;
+            for (long long k = mode + 1;; ++k) {
+                v = __dmul_rn(v, __ddiv_rn(lam, (double)k));
+                if (v < TWO_M64) break;
+                k_hi = k;
+            }
+            v = 1.0;
+            for (long long k = mode - 1; k >= 0; --k) {
+                v = __dmul_rn(v, __ddiv_rn((double)(k + 1), lam));
+                if (v < TWO_M64) break;
+                k_lo = k;
+            }
+            const uint32_t n = (uint32_t)(k_hi - k_lo + 1);
+            const uint32_t off = atomicAdd(&alloc[2 * m], n);
+            if ((int64_t)off + n > cap) atomicMin(status, PCMD_ENOMEM);
+            else {
+                double *q = qbuf + (size_t)m * cap + off;
+                q[mode - k_lo] = 1.0;
+                v = 1.0;
+                for (long long k = mode + 1; k <= k_hi; ++k) { v = __dmul_rn(v, __ddiv_rn(lam, (double)k)); q[k - k_lo] = v; }
+                v = 1.0;
+                for (long long k = mode - 1; k >= k_lo; --k) { v = __dmul_rn(v, __ddiv_rn((double)(k + 1), lam)); q[k - k_lo] = v; }
+                double S = 0.0;
+                for (uint32_t i = 0; i < n; ++i) S = __dadd_rn(S, q[i]);
+                double cs = 0.0;
+                uint32_t zeros = 0, stored = 0;
+                for (uint32_t i = 0; i < n; ++i) {      // R-C2 step 3; q[i] is no longer needed once its threshold is known
+                    cs = __dadd_rn(cs, q[i]);
+                    const unsigned long long t = __double2ull_rz(__dadd_rn(__dmul_rn(__ddiv_rn(cs, S), TWO32), 0.5));
+                    q[i] = __longlong_as_double((long long)t);
+                    if (t == 0ull) zeros++;
+                    else if (t < 4294967296ull) stored++;
+                }
+                const uint32_t dst = atomicAdd(&alloc[2 * m + 1], stored);    // stored <= n: the compact region cannot overflow if the raw one did not
+                uint32_t *out = tab_all + (size_t)m * cap;
+                uint32_t wr = dst;
+                for (uint32_t i = 0; i < n; ++i) {
+                    const unsigned long long t = (unsigned long long)__double_as_longlong(q[i]);
+                    if (t != 0ull && t < 4294967296ull) out[wr++] = (uint32_t)(t - 1ull);
+                }
+                r.k0 = (uint32_t)k_lo + zeros; r.len = stored; r.off = dst;
+                r.T0 = stored ? out[dst] : 0xFFFFFFFFu;
+                pcls = point_class(r, out);
+            }
+        }
+    }
+    if (j < Jpad) rec_out[(size_t)m * Jpad + j] = r;
+    // class of the group of four points = its most expensive point (threads 4g .. 4g+3 are neighbouring lanes)
+    pcls = min(pcls, __shfl_xor_sync(0xffffffffu, pcls, 1));
+    pcls = min(pcls, __shfl_xor_sync(0xffffffffu, pcls, 2));
+    if (j < Jpad && (j & 3) == 0) gcls_out[(size_t)m * (Jpad >> 2) + (j >> 2)] = (uint8_t)pcls;
+}
+
 // Group records at their sorted places and the padded search tables of the D classes: one warp
 // per group.  Lane w < 4 writes point w's part of the record; all lanes write the padded tables
 // (2^D words per point: the stored thresholds minus 1, then 0xFFFFFFFF).
@@ -406,18 +514,20 @@ int pcmd_build_tables(pcmd_ctx *c, const double *d_lambda, int J, int n_models, 
 }
 
 int pcmd_launch_stage1(pcmd_ctx *c, int n_models, cudaStream_t s) {
-    k_weights<<<dim3((c->Jpad + 255) / 256, n_models), 256, c->Z * sizeof(double), s>>>(
-        c->d_model, c->d_sfh, c->d_feh_grid, c->d_age_idx, c->d_feh_idx, c->d_imf_w, c->d_absmag, c->A,
-        c->Z, c->J, c->Jpad, c->B, c->mdf_cut, c->zp[0], c->zp[1], c->zp[2], c->zp[3], c->d_mdfw,
-        c->d_lambda, c->d_rec, c->d_status);
-    PCMD_LAUNCHED(c);
-    if (c->sampler_mode == 1) return pcmd_launch_agg_tables(c, n_models, s);     // no per-point tables, no work layout
-    int rc = pcmd_build_tables(c, c->d_lambda, c->J, n_models, c->d_rawcnt, c->d_klo, c->d_q, c->cap_raw,
-                          c->d_stcnt, c->d_tab, c->d_rec, c->Jpad, s);
-    if (rc) return rc;
     const int n_groups = c->Jpad >> 2;
-    k_group_classify<<<dim3((n_groups + 255) / 256, n_models), 256, 0, s>>>(c->d_rec, c->d_tab, c->cap_raw, c->Jpad,
-                                                                           c->d_gcls);
+    if (c->sampler_mode == 1) {      // aggregated sampler: lambda and fluxes only, then its own tables (agg.cu)
+        k_weights<<<dim3((c->Jpad + 255) / 256, n_models), 256, c->Z * sizeof(double), s>>>(
+            c->d_model, c->d_sfh, c->d_feh_grid, c->d_age_idx, c->d_feh_idx, c->d_imf_w, c->d_absmag, c->A,
+            c->Z, c->J, c->Jpad, c->B, c->mdf_cut, c->zp[0], c->zp[1], c->zp[2], c->zp[3], c->d_mdfw,
+            c->d_lambda, c->d_rec, c->d_status);
+        PCMD_LAUNCHED(c);
+        return pcmd_launch_agg_tables(c, n_models, s);
+    }
+    PCMD_CUDA(c, cudaMemsetAsync(c->d_alloc, 0, (size_t)n_models * 2 * sizeof(uint32_t), s));
+    k_points<<<dim3((c->Jpad + 127) / 128, n_models), 128, c->Z * sizeof(double), s>>>(
+        c->d_model, c->d_sfh, c->d_feh_grid, c->d_age_idx, c->d_feh_idx, c->d_imf_w, c->d_absmag, c->A, c->Z, c->J,
+        c->Jpad, c->B, c->mdf_cut, c->zp[0], c->zp[1], c->zp[2], c->zp[3], c->d_mdfw, c->d_lambda, c->d_q,
+        c->cap_raw, c->d_tab, c->d_alloc, c->d_rec, c->d_gcls, c->d_status);
     PCMD_LAUNCHED(c);
     k_group_sort<<<n_models, 1024, 0, s>>>(c->d_gcls, c->Jpad, c->arena_cap, c->d_gpos, c->d_plan);
     PCMD_LAUNCHED(c);
