@@ -214,10 +214,12 @@ __device__ __forceinline__ int wrap_any(int v, int N) {
 // zp - 2.5 log10(arg) for arg > 0: exponent by the add-magic-constant trick (no int->float conversion),
 // mantissa by the special-function unit, finished in one fp64 FMA
 __device__ __forceinline__ float mag_of(float arg, double zp) {
-    const uint32_t bits = __float_as_uint(arg);
+    // branch-free: the 16 magnitudes of a thread are independent chains the scheduler can interleave
+    const uint32_t bits = __float_as_uint(fmaxf(arg, 1.17549435e-38f));
     const float e = __uint_as_float(0x4B000000u | (bits >> 23)) - 8388735.0f;      // (2^23 + biased exponent) - 2^23 - 127
     const float mant = __uint_as_float((bits & 0x007FFFFFu) | 0x3F800000u);
-    return (float)fma((double)(e + __log2f(mant)), -0.75257498915995298, zp);
+    const float mg = (float)fma((double)(e + __log2f(mant)), -0.75257498915995298, zp);
+    return arg > 0.f ? mg : __int_as_float(0x7fc00000);
 }
 __device__ __forceinline__ float sqrt_approx(float x) {
     float r;
@@ -255,11 +257,12 @@ __device__ __forceinline__ float noise_mag_one(const Cv2Args &a, float Gi, uint3
         const float var = (a.shot_noise ? fmaxf(Gi + skyf, 0.f) : 0.f) + rs2;
         arg = Gi + sqrt_approx(var) * g;
     }
-    return (arg > 0.f) ? mag_of(arg, a.zp) : __int_as_float(0x7fc00000);
+    return mag_of(arg, a.zp);
 }
 
-template <int K, bool VEC>
-__global__ void __launch_bounds__(C2_THREADS, 4) k_conv2(const Cv2Args a) {
+// NOISE = false: no shot / read noise and no Poisson sky (stage 5 is the magnitude only): a leaner instance
+template <int K, bool VEC, bool NOISE>
+__global__ void __launch_bounds__(C2_THREADS, ((K <= 7 && !NOISE) ? 5 : 4)) k_conv2(const Cv2Args a) {
     constexpr int R = (K - 1) / 2, RA = (R + 3) & ~3, OFF = RA - R;
     constexpr int SW = C2_TW + 2 * RA;            // halo-tile row stride (floats), a multiple of 4
     constexpr int SH = C2_TH + K - 1;             // halo-tile rows
@@ -272,7 +275,7 @@ __global__ void __launch_bounds__(C2_THREADS, 4) k_conv2(const Cv2Args a) {
     const int N = a.N, m = blockIdx.z, mb = m * a.B + a.band, tid = threadIdx.x;
     const float *F = a.F + (size_t)mb * a.P;
     const int x0 = blockIdx.x * C2_TW, y0 = blockIdx.y * C2_TH;
-    const bool psky = a.poisson_sky && a.sky > 0.0;
+    const bool psky = NOISE && a.poisson_sky && a.sky > 0.0;
     int sky_d = -1;                                // log2 of the padded sky table in shared memory; -1: table stays in global memory
     if (psky && a.sky_rec.len < SKY_CAP) {
         sky_d = 32 - __clz(a.sky_rec.len);         // 2^sky_d > len: at least one 0xFFFFFFFF pad entry
@@ -284,23 +287,15 @@ __global__ void __launch_bounds__(C2_THREADS, 4) k_conv2(const Cv2Args a) {
     // one conditional add / subtract wraps an index when the image is at least as large as the halo tile
     const bool big = N >= SW && N >= SH;
     if (VEC) {
-        constexpr int NQ = SW / 4;                 // 16-byte segments per halo row (18 ... 22): one lane each
-        const int lane = tid & 31, wrp = tid >> 5;
-        if (lane < NQ) {
-            int gx = x0 - RA + 4 * lane;           // N % 4 == 0: a segment never straddles the edge
-            if (big) { gx += gx < 0 ? N : 0; gx -= gx >= N ? N : 0; } else gx = wrap_any(gx, N);
-            int gy = y0 - R + wrp;
-            if (big) gy += gy < 0 ? N : 0; else gy = wrap_any(gy, N);
-            const float *src = F + gx;
-            uint32_t dst = (uint32_t)__cvta_generic_to_shared(reinterpret_cast<float4 *>(tile) + wrp * NQ + lane);
-#pragma unroll
-            for (int it = 0; it < (SH + C2_THREADS / 32 - 1) / (C2_THREADS / 32); ++it) {      // all copies in flight at once
-                if (wrp + it * (C2_THREADS / 32) < rows_used) {
-                    if (big) gy -= gy >= N ? N : 0; else gy = wrap_any(gy, N);
-                    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src + (size_t)gy * N) : "memory");
-                    gy += C2_THREADS / 32; dst += (C2_THREADS / 32) * NQ * 16;
-                }
-            }
+        constexpr int NQ = SW / 4;                 // 16-byte segments per halo row (18 ... 22)
+        // N % 4 == 0: a segment never straddles the edge.  Flat index over (row, segment): every lane copies
+        for (int t = tid; t < rows_used * NQ; t += C2_THREADS) {
+            const int i = t / NQ, q = t - i * NQ;
+            int gy = y0 - R + i, gx = x0 - RA + 4 * q;
+            if (big) { gy += gy < 0 ? N : 0; gy -= gy >= N ? N : 0; gx += gx < 0 ? N : 0; gx -= gx >= N ? N : 0; }
+            else { gy = wrap_any(gy, N); gx = wrap_any(gx, N); }
+            const uint32_t dst = (uint32_t)__cvta_generic_to_shared(reinterpret_cast<float4 *>(tile) + t);
+            asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(F + (size_t)gy * N + gx) : "memory");
         }
         asm volatile("cp.async.wait_all;" ::: "memory");
     } else {
@@ -355,7 +350,7 @@ __global__ void __launch_bounds__(C2_THREADS, 4) k_conv2(const Cv2Args a) {
     // ---- stage 5 on the 16 outputs
     const uint32_t mctr = a.model0 + (uint32_t)m;
     const float skyf = (float)a.sky, rs2 = (float)(a.read_sigma * a.read_sigma);
-    const bool need_g = a.shot_noise || a.read_sigma > 0.0;
+    const bool need_g = NOISE && (a.shot_noise || a.read_sigma > 0.0);
     const uint32_t *stab = sky_d >= 0 ? ssky : a.sky_tab + a.sky_rec.off;
     const int x = x0 + 4 * xg, yt = y0 + 4 * yb;
     if (x >= N || yt >= N) return;
@@ -367,17 +362,17 @@ __global__ void __launch_bounds__(C2_THREADS, 4) k_conv2(const Cv2Args a) {
             for (int j = 0; j < 4; ++j)
                 *reinterpret_cast<float4 *>(a.tap_conv + (size_t)mb * a.P + p0 + (size_t)j * N) = make_float4(acc[j][0], acc[j][1], acc[j][2], acc[j][3]);
         }
-        if (!need_g && !psky) {
+        if (!NOISE) {
 #pragma unroll
             for (int j = 0; j < 4; ++j) {
                 float mg[4];
 #pragma unroll
-                for (int c = 0; c < 4; ++c) mg[c] = (acc[j][c] > 0.f) ? mag_of(acc[j][c], a.zp) : __int_as_float(0x7fc00000);
+                for (int c = 0; c < 4; ++c) mg[c] = mag_of(acc[j][c], a.zp);
                 *reinterpret_cast<float4 *>(mag + (size_t)j * N) = make_float4(mg[0], mg[1], mg[2], mg[3]);
             }
         } else {
-#pragma unroll
-            for (int j = 0; j < 4; ++j) {
+#pragma unroll 1
+            for (int j = 0; j < 4; ++j) {       // one row of four pixels at a time: sixteen interleaved Philox calls would spill
                 float mg[4];
 #pragma unroll
                 for (int c = 0; c < 4; ++c)
@@ -411,16 +406,21 @@ static cudaError_t conv2_launch(const Cv2Args &a, int n_models, cudaStream_t s) 
     const dim3 grid((a.N + C2_TW - 1) / C2_TW, (a.N + C2_TH - 1) / C2_TH, n_models);
     const bool vec = (a.N & 3) == 0 && ((reinterpret_cast<uintptr_t>(a.F) | reinterpret_cast<uintptr_t>(a.mag) |
                                          reinterpret_cast<uintptr_t>(a.tap_conv)) & 15) == 0;
-    if (vec) k_conv2<K, true><<<grid, C2_THREADS, conv2_smem<K>(), s>>>(a);
-    else k_conv2<K, false><<<grid, C2_THREADS, conv2_smem<K>(), s>>>(a);
+    const bool noise = a.shot_noise || a.read_sigma > 0.0 || (a.poisson_sky && a.sky > 0.0);
+    if (vec && noise) k_conv2<K, true, true><<<grid, C2_THREADS, conv2_smem<K>(), s>>>(a);
+    else if (vec) k_conv2<K, true, false><<<grid, C2_THREADS, conv2_smem<K>(), s>>>(a);
+    else if (noise) k_conv2<K, false, true><<<grid, C2_THREADS, conv2_smem<K>(), s>>>(a);
+    else k_conv2<K, false, false><<<grid, C2_THREADS, conv2_smem<K>(), s>>>(a);
     return cudaGetLastError();
 }
 
 // opt-in to > 48 KB of dynamic shared memory (once per ctx, i.e. per device)
 int pcmd_conv_setup(pcmd_ctx *c) {
 #define C2_OPT(K)                                                                                                    \
-    PCMD_CUDA(c, cudaFuncSetAttribute(k_conv2<K, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)conv2_smem<K>())); \
-    PCMD_CUDA(c, cudaFuncSetAttribute(k_conv2<K, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)conv2_smem<K>()));
+    PCMD_CUDA(c, cudaFuncSetAttribute(k_conv2<K, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)conv2_smem<K>())); \
+    PCMD_CUDA(c, cudaFuncSetAttribute(k_conv2<K, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)conv2_smem<K>())); \
+    PCMD_CUDA(c, cudaFuncSetAttribute(k_conv2<K, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)conv2_smem<K>())); \
+    PCMD_CUDA(c, cudaFuncSetAttribute(k_conv2<K, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)conv2_smem<K>()));
     C2_OPT(5) C2_OPT(7) C2_OPT(15) C2_OPT(21)
 #undef C2_OPT
     return PCMD_OK;

@@ -12,11 +12,6 @@
 // barrier inside the stream -- and writes one partial flux per (tile fragment, band, pixel);
 // k_reduce_dust adds the (at most a few) fragments of a tile.
 #include "pcmd_internal.cuh"
-#ifdef S2_TIMES
-#include <vector>
-#include <stdio.h>
-#include <stdlib.h>
-#endif
 
 #ifndef S2_THREADS
 #define S2_THREADS 256
@@ -53,9 +48,6 @@ struct S2Args {
     int32_t *counter;        // work-unit counter, zeroed before the launch
     uint64_t *hash;          // optional [n_models][P], zeroed before the launch
     uint32_t *total;         // optional [n_models][P], zeroed before the launch
-#ifdef S2_TIMES
-    long long *times;
-#endif
 };
 
 // ---- bulk async copy (TMA) + mbarrier ---------------------------------------------------------
@@ -490,11 +482,6 @@ __global__ void __launch_bounds__(S2_THREADS, S2_MINB) k_stage2(const S2Args a) 
         }
     }
     __syncthreads();
-#ifdef S2_TIMES
-    if (threadIdx.x == 0) { long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); a.times[2 * blockIdx.x] = t; }
-    unsigned smid; asm volatile("mov.u32 %0, %%smid;" : "=r"(smid));
-    long long dbg_wait = 0, dbg_prod = 0; const long long dbg_t0 = clock64();
-#endif
     S2State<NB, COUNTS> st;
     uint32_t pix[S2_PX];
     PhiloxPix ph[S2_PX];                 // the group-independent part of the Philox rounds, per pixel
@@ -503,13 +490,7 @@ __global__ void __launch_bounds__(S2_THREADS, S2_MINB) k_stage2(const S2Args a) 
     int s = 0, sp = 0;
     uint32_t par = 0, parp = 0;
     for (int q = 0;; ++q) {
-#ifdef S2_TIMES
-        const long long tw0 = clock64();
-#endif
         mbar_wait(&sh.full[s], par);
-#ifdef S2_TIMES
-        dbg_wait += clock64() - tw0;
-#endif
         const ChunkDesc d = sh.desc[s];
         const int mt = d.m * a.mts;
         if (d.flags & S2_F_FIRST) {
@@ -577,18 +558,12 @@ __global__ void __launch_bounds__(S2_THREADS, S2_MINB) k_stage2(const S2Args a) 
             }
         }
         if (d.flags & S2_F_END) {
-#ifdef S2_TIMES
-            if (lane == 0) { long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); const int wi = blockIdx.x * S2_WARPS + (threadIdx.x >> 5); a.times[2 * gridDim.x + wi] = t; a.times[(2 + S2_WARPS) * gridDim.x + 3 * wi] = dbg_wait; a.times[(2 + S2_WARPS) * gridDim.x + 3 * wi + 1] = dbg_prod; a.times[(2 + S2_WARPS) * gridDim.x + 3 * wi + 2] = clock64() - dbg_t0; if (threadIdx.x == 0) a.times[2 * blockIdx.x + 1] = smid; }
-#endif
             break;
         }
         // Producer turn q (after chunk q >= 1): chunk q-1's stage, which every warp has normally left long ago,
         // takes chunk q-1+S2_NST.  The turns rotate over the warps (no warp is slowed more than the others, nobody
         // waits for a producer warp) and run in order (ticket).
         if (q >= 1 && ((q - 1) & (S2_WARPS - 1)) == wid) {
-#ifdef S2_TIMES
-            const long long tp0 = clock64();
-#endif
             while (lds_acquire_u32(&sh.ticket) != (uint32_t)(q - 1)) { }
             __threadfence_block();
             if (lds_acquire_u32(&sh.live)) {
@@ -597,9 +572,6 @@ __global__ void __launch_bounds__(S2_THREADS, S2_MINB) k_stage2(const S2Args a) 
             }
             __threadfence_block();
             sts32(lead, &sh.ticket, q);
-#ifdef S2_TIMES
-            dbg_prod += clock64() - tp0;
-#endif
         }
         sp = s; parp = par;
         if (++s == S2_NST) { s = 0; par ^= 1u; }
@@ -690,11 +662,6 @@ int pcmd_launch_stage2(pcmd_ctx *c, int n_models, uint64_t seed, uint32_t model0
     const int64_t n_units = (int64_t)n_models * a.n_tiles * a.n_seg;
     const int64_t slots = (int64_t)c->sm_count * (d_hash ? 1 : c->s2_ctas_per_sm);
     const int grid = (int)(n_units < slots ? n_units : slots);
-#ifdef S2_TIMES
-    static long long *d_times = nullptr;
-    if (!d_times) cudaMalloc(&d_times, (size_t)grid * (2 + 4 * S2_WARPS) * sizeof(long long));
-    a.times = d_times;
-#endif
     cudaError_t e;
     const bool counts = d_hash != nullptr;
     if (c->B <= 2) e = launch_s2<2>(a, counts, grid, s);
@@ -714,14 +681,6 @@ int pcmd_launch_stage2(pcmd_ctx *c, int n_models, uint64_t seed, uint32_t model0
     const int64_t n = c->P * n_models;
     k_reduce_dust<<<(unsigned)((n + 255) / 256), 256, 0, s>>>(r);
     PCMD_LAUNCHED(c);
-#ifdef S2_TIMES
-    if (getenv("S2_TIMES_FILE")) {
-        cudaStreamSynchronize(s);
-        std::vector<long long> h((size_t)grid * (2 + 4 * S2_WARPS));
-        cudaMemcpy(h.data(), d_times, h.size() * sizeof(long long), cudaMemcpyDeviceToHost);
-        FILE *f = fopen(getenv("S2_TIMES_FILE"), "wb"); fwrite(h.data(), sizeof(long long), h.size(), f); fclose(f);
-    }
-#endif
     return PCMD_OK;
 }
 
