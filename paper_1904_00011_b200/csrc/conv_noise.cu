@@ -191,6 +191,9 @@ __device__ __forceinline__ void noise_mag_epilogue(const CvArgs &a, const float 
 #define C2_TH 64
 #define C2_THREADS 256
 #define C2_KMAX 21
+#ifndef C2_MINB_CLEAN
+#define C2_MINB_CLEAN 5       // CTAs per SM of the noise-free instances (register cap 51)
+#endif
 
 struct Cv2Args {
     const float *F;      // [n_models][B][P] dusty flux
@@ -204,7 +207,26 @@ struct Cv2Args {
     uint32_t key0, key1, model0;
     double zp, sky, read_sigma;
     float fr[C2_KMAX], fc[C2_KMAX];    // row factor, column factor of this band
+    float2 rp[C2_KMAX];                // rp[t] = (fr[t], fr[t-1]): coefficient pair of an aligned input pair in the row pass
+    float2 cp[C2_KMAX];                // cp[k] = (fc[k], fc[k]): coefficient pair of an output pair in the column pass
 };
+
+// packed FP32 pairs (FFMA2 on sm_100a: two FMAs per instruction, half the issue slots of the two passes)
+typedef unsigned long long f32x2;
+__device__ __forceinline__ f32x2 pack2(float lo, float hi) {
+    f32x2 r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+    return r;
+}
+__device__ __forceinline__ void unpack2(f32x2 v, float &lo, float &hi) {
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
+}
+__device__ __forceinline__ f32x2 fma2(f32x2 a, f32x2 b, f32x2 c) {      // a * b + c, lane-wise
+    f32x2 r;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c));
+    return r;
+}
+__device__ __forceinline__ f32x2 as_pair(const float2 &p) { return *reinterpret_cast<const f32x2 *>(&p); }
 
 __device__ __forceinline__ int wrap_any(int v, int N) {
     v %= N;
@@ -262,7 +284,7 @@ __device__ __forceinline__ float noise_mag_one(const Cv2Args &a, float Gi, uint3
 
 // NOISE = false: no shot / read noise and no Poisson sky (stage 5 is the magnitude only): a leaner instance
 template <int K, bool VEC, bool NOISE>
-__global__ void __launch_bounds__(C2_THREADS, ((K <= 7 && !NOISE) ? 5 : 4)) k_conv2(const Cv2Args a) {
+__global__ void __launch_bounds__(C2_THREADS, (NOISE ? 4 : C2_MINB_CLEAN)) k_conv2(const Cv2Args a) {
     constexpr int R = (K - 1) / 2, RA = (R + 3) & ~3, OFF = RA - R;
     constexpr int SW = C2_TW + 2 * RA;            // halo-tile row stride (floats), a multiple of 4
     constexpr int SH = C2_TH + K - 1;             // halo-tile rows
@@ -270,8 +292,8 @@ __global__ void __launch_bounds__(C2_THREADS, ((K <= 7 && !NOISE) ? 5 : 4)) k_co
     constexpr int SKY_CAP = 1024;                 // Poisson-sky thresholds kept in shared memory
     extern __shared__ __align__(16) float sm[];
     float *tile = sm;                             // [SH][SW]
-    float *hrow = sm + SH * SW;                   // [SH][C2_TW]
-    uint32_t *ssky = reinterpret_cast<uint32_t *>(hrow + SH * C2_TW);   // [SKY_CAP]
+    float *hrow = sm;                             // row results overwrite the first 64 columns of their own tile row (stride SW)
+    uint32_t *ssky = reinterpret_cast<uint32_t *>(sm + SH * SW);        // [SKY_CAP], noisy instances only
     const int N = a.N, m = blockIdx.z, mb = m * a.B + a.band, tid = threadIdx.x;
     const float *F = a.F + (size_t)mb * a.P;
     const int x0 = blockIdx.x * C2_TW, y0 = blockIdx.y * C2_TH;
@@ -288,14 +310,28 @@ __global__ void __launch_bounds__(C2_THREADS, ((K <= 7 && !NOISE) ? 5 : 4)) k_co
     const bool big = N >= SW && N >= SH;
     if (VEC) {
         constexpr int NQ = SW / 4;                 // 16-byte segments per halo row (18 ... 22)
-        // N % 4 == 0: a segment never straddles the edge.  Flat index over (row, segment): every lane copies
-        for (int t = tid; t < rows_used * NQ; t += C2_THREADS) {
-            const int i = t / NQ, q = t - i * NQ;
-            int gy = y0 - R + i, gx = x0 - RA + 4 * q;
-            if (big) { gy += gy < 0 ? N : 0; gy -= gy >= N ? N : 0; gx += gx < 0 ? N : 0; gx -= gx >= N ? N : 0; }
-            else { gy = wrap_any(gy, N); gx = wrap_any(gx, N); }
-            const uint32_t dst = (uint32_t)__cvta_generic_to_shared(reinterpret_cast<float4 *>(tile) + t);
-            asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(F + (size_t)gy * N + gx) : "memory");
+        // N % 4 == 0: a segment never straddles the edge.  Flat index over (row, segment): every lane copies.
+        if (big) {      // (row, segment) and the wrapped source row advance incrementally: no division, no modulo
+            constexpr int DI = C2_THREADS / NQ, DQ = C2_THREADS - DI * NQ;
+            const int i0 = tid / NQ;
+            int q = tid - i0 * NQ, gx4 = x0 - RA + 4 * q, gy = y0 - R + i0;
+            gy += gy < 0 ? N : 0; gy -= gy >= N ? N : 0;
+            uint32_t dst = (uint32_t)__cvta_generic_to_shared(reinterpret_cast<float4 *>(tile) + tid);
+            for (int t = tid; t < rows_used * NQ; t += C2_THREADS) {
+                int gx = gx4;
+                gx += gx < 0 ? N : 0; gx -= gx >= N ? N : 0;
+                asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(F + ((size_t)(uint32_t)(gy * N + gx))) : "memory");
+                dst += C2_THREADS * 16; q += DQ; gx4 += 4 * DQ; gy += DI;
+                if (q >= NQ) { q -= NQ; gx4 -= 4 * NQ; gy += 1; }
+                gy -= gy >= N ? N : 0;
+            }
+        } else {
+            for (int t = tid; t < rows_used * NQ; t += C2_THREADS) {
+                const int i = t / NQ, q = t - i * NQ;
+                const int gy = wrap_any(y0 - R + i, N), gx = wrap_any(x0 - RA + 4 * q, N);
+                const uint32_t dst = (uint32_t)__cvta_generic_to_shared(reinterpret_cast<float4 *>(tile) + t);
+                asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(F + (size_t)gy * N + gx) : "memory");
+            }
         }
         asm volatile("cp.async.wait_all;" ::: "memory");
     } else {
@@ -311,41 +347,61 @@ __global__ void __launch_bounds__(C2_THREADS, ((K <= 7 && !NOISE) ? 5 : 4)) k_co
     for (int it = 0; it < ROW_IT; ++it) {
         const int t = tid + it * C2_THREADS;
         const int i = t / (C2_TW / 4), sgm = t - i * (C2_TW / 4);
-        if (i >= rows_used) break;
+        const bool live = i < rows_used;        // a warp holds two rows: both halves reach the __syncwarp below
         float v[NV * 4];
 #pragma unroll
         for (int q = 0; q < NV; ++q) {
-            const float4 f4 = reinterpret_cast<const float4 *>(tile + i * SW)[sgm + q];
+            const float4 f4 = live ? reinterpret_cast<const float4 *>(tile + i * SW)[sgm + q] : make_float4(0.f, 0.f, 0.f, 0.f);
             v[4 * q] = f4.x; v[4 * q + 1] = f4.y; v[4 * q + 2] = f4.z; v[4 * q + 3] = f4.w;
         }
-        float h[4] = {0.f, 0.f, 0.f, 0.f};
+        // h[c] = sum_i fr[b - i] v[i], i = OFF + c ... OFF + c + K - 1, b = OFF + c + K - 1: aligned input pairs
+        // (v[2m], v[2m+1]) take the coefficient pair rp[b - 2m] in one FFMA2, the odd end(s) a plain FMA
+        float h[4];
 #pragma unroll
-        for (int k = 0; k < K; ++k)
+        for (int c = 0; c < 4; ++c) {
+            constexpr int dummy = 0; (void)dummy;
+            const int lo = OFF + c, hi = OFF + c + K - 1;
+            f32x2 acc2 = pack2(0.f, 0.f);
+            float single = 0.f;
 #pragma unroll
-            for (int c = 0; c < 4; ++c) h[c] = fmaf(a.fr[k], v[OFF + c + (K - 1) - k], h[c]);
-        reinterpret_cast<float4 *>(hrow + i * C2_TW)[sgm] = make_float4(h[0], h[1], h[2], h[3]);
+            for (int i = lo; i <= hi; ++i) {
+                if ((i & 1) == 0 && i + 1 <= hi) acc2 = fma2(pack2(v[i], v[i + 1]), as_pair(a.rp[hi - i]), acc2);
+                else if ((i & 1) == 1 && i == lo) single = fmaf(a.fr[hi - i], v[i], single);
+                else if ((i & 1) == 0 && i == hi) single = fmaf(a.fr[0], v[i], single);
+            }
+            float p0, p1;
+            unpack2(acc2, p0, p1);
+            h[c] = (p0 + p1) + single;
+        }
+        // in place: the 16 tasks of a row sit in one warp; every lane has its window in registers before any lane stores
+        __syncwarp();
+        if (live) reinterpret_cast<float4 *>(hrow + i * SW)[sgm] = make_float4(h[0], h[1], h[2], h[3]);
     }
     __syncthreads();
     // ---- column pass: G[y][x] = sum_k fc[k] h[y - (k - R)][x], 4 x 4 outputs per thread
     const int xg = tid & 15, yb = tid >> 4;
     float acc[4][4];
+    {
+        f32x2 a01[4], a23[4];
 #pragma unroll
-    for (int j = 0; j < 4; ++j)
+        for (int j = 0; j < 4; ++j) { a01[j] = pack2(0.f, 0.f); a23[j] = pack2(0.f, 0.f); }
+        if (y0 + 4 * yb < N) {
 #pragma unroll
-        for (int c = 0; c < 4; ++c) acc[j][c] = 0.f;
-    if (y0 + 4 * yb < N) {
+            for (int n = 0; n < K + 3; ++n) {
+                const float4 hv = reinterpret_cast<const float4 *>(hrow + (4 * yb + n) * SW)[xg];
+                const f32x2 h01 = pack2(hv.x, hv.y), h23 = pack2(hv.z, hv.w);
 #pragma unroll
-        for (int n = 0; n < K + 3; ++n) {
-            const float4 hv = reinterpret_cast<const float4 *>(hrow + (4 * yb + n) * C2_TW)[xg];
-#pragma unroll
-            for (int j = 0; j < 4; ++j) {
-                const int k = j + (K - 1) - n;
-                if (k >= 0 && k < K) {
-                    acc[j][0] = fmaf(a.fc[k], hv.x, acc[j][0]); acc[j][1] = fmaf(a.fc[k], hv.y, acc[j][1]);
-                    acc[j][2] = fmaf(a.fc[k], hv.z, acc[j][2]); acc[j][3] = fmaf(a.fc[k], hv.w, acc[j][3]);
+                for (int j = 0; j < 4; ++j) {
+                    const int k = j + (K - 1) - n;
+                    if (k >= 0 && k < K) {
+                        a01[j] = fma2(h01, as_pair(a.cp[k]), a01[j]);
+                        a23[j] = fma2(h23, as_pair(a.cp[k]), a23[j]);
+                    }
                 }
             }
         }
+#pragma unroll
+        for (int j = 0; j < 4; ++j) { unpack2(a01[j], acc[j][0], acc[j][1]); unpack2(a23[j], acc[j][2], acc[j][3]); }
     }
     // ---- stage 5 on the 16 outputs
     const uint32_t mctr = a.model0 + (uint32_t)m;
@@ -396,9 +452,9 @@ __global__ void __launch_bounds__(C2_THREADS, ((K <= 7 && !NOISE) ? 5 : 4)) k_co
 }
 
 template <int K>
-static size_t conv2_smem() {
+static size_t conv2_smem(bool noise) {
     constexpr int R = (K - 1) / 2, RA = (R + 3) & ~3;
-    return ((size_t)(C2_TH + K - 1) * (C2_TW + 2 * RA) + (size_t)(C2_TH + K - 1) * C2_TW + 1024) * sizeof(float);
+    return ((size_t)(C2_TH + K - 1) * (C2_TW + 2 * RA) + (noise ? 1024 : 0)) * sizeof(float);
 }
 
 template <int K>
@@ -407,24 +463,14 @@ static cudaError_t conv2_launch(const Cv2Args &a, int n_models, cudaStream_t s) 
     const bool vec = (a.N & 3) == 0 && ((reinterpret_cast<uintptr_t>(a.F) | reinterpret_cast<uintptr_t>(a.mag) |
                                          reinterpret_cast<uintptr_t>(a.tap_conv)) & 15) == 0;
     const bool noise = a.shot_noise || a.read_sigma > 0.0 || (a.poisson_sky && a.sky > 0.0);
-    if (vec && noise) k_conv2<K, true, true><<<grid, C2_THREADS, conv2_smem<K>(), s>>>(a);
-    else if (vec) k_conv2<K, true, false><<<grid, C2_THREADS, conv2_smem<K>(), s>>>(a);
-    else if (noise) k_conv2<K, false, true><<<grid, C2_THREADS, conv2_smem<K>(), s>>>(a);
-    else k_conv2<K, false, false><<<grid, C2_THREADS, conv2_smem<K>(), s>>>(a);
+    if (vec && noise) k_conv2<K, true, true><<<grid, C2_THREADS, conv2_smem<K>(true), s>>>(a);
+    else if (vec) k_conv2<K, true, false><<<grid, C2_THREADS, conv2_smem<K>(false), s>>>(a);
+    else if (noise) k_conv2<K, false, true><<<grid, C2_THREADS, conv2_smem<K>(true), s>>>(a);
+    else k_conv2<K, false, false><<<grid, C2_THREADS, conv2_smem<K>(false), s>>>(a);
     return cudaGetLastError();
 }
 
-// opt-in to > 48 KB of dynamic shared memory (once per ctx, i.e. per device)
-int pcmd_conv_setup(pcmd_ctx *c) {
-#define C2_OPT(K)                                                                                                    \
-    PCMD_CUDA(c, cudaFuncSetAttribute(k_conv2<K, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)conv2_smem<K>())); \
-    PCMD_CUDA(c, cudaFuncSetAttribute(k_conv2<K, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)conv2_smem<K>())); \
-    PCMD_CUDA(c, cudaFuncSetAttribute(k_conv2<K, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)conv2_smem<K>())); \
-    PCMD_CUDA(c, cudaFuncSetAttribute(k_conv2<K, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)conv2_smem<K>()));
-    C2_OPT(5) C2_OPT(7) C2_OPT(15) C2_OPT(21)
-#undef C2_OPT
-    return PCMD_OK;
-}
+int pcmd_conv_setup(pcmd_ctx *) { return PCMD_OK; }     // k_conv2 needs at most 33 KB of dynamic shared memory: no opt-in
 
 static int launch_conv2(pcmd_ctx *c, int n_models, uint64_t seed, uint32_t model0, float *d_mag, const float *h_fac,
                         cudaStream_t s) {
@@ -437,6 +483,10 @@ static int launch_conv2(pcmd_ctx *c, int n_models, uint64_t seed, uint32_t model
         for (int k = 0; k < C2_KMAX; ++k) {
             a.fr[k] = k < c->K ? h_fac[((size_t)b * 2) * c->K + k] : 0.f;
             a.fc[k] = k < c->K ? h_fac[((size_t)b * 2 + 1) * c->K + k] : 0.f;
+        }
+        for (int k = 0; k < C2_KMAX; ++k) {
+            a.rp[k] = make_float2(a.fr[k], k > 0 ? a.fr[k - 1] : 0.f);
+            a.cp[k] = make_float2(a.fc[k], a.fc[k]);
         }
         cudaError_t e;
         switch (c->K) {
