@@ -34,7 +34,7 @@ extern "C" const char *pcmd_strerror(int code) {
 
 static void free_scratch(pcmd_ctx *c) {
     cudaFree(c->d_sfh); cudaFree(c->d_model); cudaFree(c->d_mdfw); cudaFree(c->d_lambda);
-    cudaFree(c->d_rawcnt); cudaFree(c->d_klo); cudaFree(c->d_q); cudaFree(c->d_stcnt);
+    cudaFree(c->d_q);
     cudaFree(c->d_tab); cudaFree(c->d_rec); cudaFree(c->d_grp); cudaFree(c->d_plan);
     cudaFree(c->d_gcls); cudaFree(c->d_arena); cudaFree(c->d_gpos); cudaFree(c->d_alloc); c->d_alloc = nullptr;
     c->d_grp = nullptr; c->d_plan = nullptr; c->d_gcls = nullptr; c->d_arena = nullptr; c->d_gpos = nullptr;
@@ -45,7 +45,7 @@ static void free_scratch(pcmd_ctx *c) {
     c->agg_tcap = 0; c->agg_models = 0;
     if (c->h_stage) cudaFreeHost(c->h_stage);
     c->d_sfh = nullptr; c->d_model = nullptr; c->d_mdfw = nullptr; c->d_lambda = nullptr;
-    c->d_rawcnt = nullptr; c->d_klo = nullptr; c->d_q = nullptr; c->d_stcnt = nullptr;
+    c->d_q = nullptr;
     c->d_tab = nullptr; c->d_rec = nullptr; c->h_stage = nullptr;
     c->cap_models = 0; c->cap_raw = 0;
 }
@@ -63,9 +63,6 @@ static int ensure_scratch(pcmd_ctx *c, int n_models, int64_t cap_raw, int64_t ag
     PCMD_CUDA(c, cudaMalloc(&c->d_model, (size_t)nm * sizeof(DevModel)));
     PCMD_CUDA(c, cudaMalloc(&c->d_mdfw, (size_t)nm * c->Z * sizeof(double)));
     PCMD_CUDA(c, cudaMalloc(&c->d_lambda, (size_t)nm * J * sizeof(double)));
-    PCMD_CUDA(c, cudaMalloc(&c->d_rawcnt, (size_t)nm * (J + 1) * sizeof(uint32_t)));
-    PCMD_CUDA(c, cudaMalloc(&c->d_stcnt, (size_t)nm * (J + 1) * sizeof(uint32_t)));
-    PCMD_CUDA(c, cudaMalloc(&c->d_klo, (size_t)nm * J * sizeof(uint32_t)));
     PCMD_CUDA(c, cudaMalloc(&c->d_alloc, (size_t)nm * 2 * sizeof(uint32_t)));
     PCMD_CUDA(c, cudaMalloc(&c->d_q, (size_t)nm * cr * sizeof(double)));
     PCMD_CUDA(c, cudaMalloc(&c->d_tab, (size_t)nm * cr * sizeof(uint32_t)));

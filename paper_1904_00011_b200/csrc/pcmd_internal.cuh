@@ -17,9 +17,10 @@ struct __align__(16) PointRec {
 
 // Stage-2 work layout.  Groups of four consecutive isochrone points (one
 // Philox call, R-C1) are classified by how many sampler thresholds decide almost every draw and
-// sorted by class; a class is cut into chunks (the unit of shared-memory staging); the chunks of all
-// (model, pixel tile) pairs form one cost-weighted sequence that is cut into equal shares, one per
-// persistent CTA (no work queue, no atomics).
+// sorted by class; a class is cut into chunks (the unit of shared-memory staging); a model's chunk list
+// is cut by estimated cost into n_seg segments, and a work unit = (model, 512-pixel tile, segment).
+// Persistent CTAs take units from an atomic counter (units are fixed, so results do not depend on which
+// CTA ran them) and stream their chunks through a shared-memory ring.
 #define S2_NCLASS 10       // classes, most expensive first:
 #define S2_CLS_D9 1        //   0 bisection in global memory (tables longer than 511)
 #define S2_CLS_D7 2        //   1-3 branch-free search of a padded table of 2^D words in shared memory
@@ -35,7 +36,7 @@ struct __align__(16) PointRec {
 #ifndef S2_TABW
 #define S2_TABW 4096        // words of staged search tables per chunk (16 KB): 32 / 8 / 2 groups of D5 / D7 / D9
 #endif
-// cost model of the static partition: ~SM cycles per warp and group of each class loop (profiles/), and per chunk
+// cost model of the segment cut: ~SM cycles per warp and group of each class loop (profiles/), and per chunk
 #define S2_COST_G 1500u
 #define S2_COST_D9 420u
 #define S2_COST_D7 340u
@@ -114,11 +115,8 @@ struct pcmd_ctx {
     int stage_flip;
     double *d_mdfw;        // [cap_models][Z]
     double *d_lambda;      // [cap_models][J]
-    uint32_t *d_rawcnt;    // [cap_models][J+1] raw table range sizes -> exclusive offsets
     uint32_t *d_alloc;     // [cap_models][2] bump allocators of the raw and the compact table regions (k_points)
-    uint32_t *d_klo;       // [cap_models][J]
     double *d_q;           // [cap_models][cap_raw] pmf ratios, then thresholds (as uint64)
-    uint32_t *d_stcnt;     // [cap_models][J+1] stored counts -> exclusive offsets
     uint32_t *d_tab;       // [cap_models][cap_raw] stored thresholds minus 1
     PointRec *d_rec;       // [cap_models][Jpad]
     float *d_fdust; int64_t fdust_elems;   // [realisations][B][P] dusty flux

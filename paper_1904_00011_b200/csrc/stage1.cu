@@ -202,6 +202,8 @@ __global__ void k_table_compact(int J, int n_models, const uint32_t *__restrict_
 // lay out the padded search tables of the D classes.  One block per model.
 // Class of a point:  L1/L2/L4: k0 = 0 and the probability of more than L stars is below 2^-10
 // (its (L+1)-th threshold is above 2^32 (1 - 2^-10)): L inline compares decide the draw;
+// S3/S4: k0 = 0 and more than 7 / 15 stars have probability below 2^-10: the first 2^D - 1 thresholds are
+// searched branch-free in shared memory, the overflow path finishes the rest;
 // D5/D7/D9: table of at most 2^D - 1 thresholds, searched branch-free in shared memory;
 // class 0: longer tables, bisection in global memory.  A group takes the most expensive class
 // of its four points.
@@ -229,21 +231,6 @@ __device__ __forceinline__ int point_class(const PointRec &r, const uint32_t *__
     if (r.len <= 127) return S2_CLS_D7;
     if (r.len <= 511) return S2_CLS_D9;
     return 0;
-}
-
-// Class of every group: one thread per group.
-__global__ void __launch_bounds__(256) k_group_classify(const PointRec *__restrict__ rec_all,
-                                                        const uint32_t *__restrict__ tab_all, int64_t cap, int Jpad,
-                                                        uint8_t *__restrict__ cls_all) {
-    const int m = blockIdx.y, n_groups = Jpad >> 2;
-    const int g = blockIdx.x * blockDim.x + threadIdx.x;
-    if (g >= n_groups) return;
-    const PointRec *rec = rec_all + (size_t)m * Jpad;
-    const uint32_t *tab = tab_all + (size_t)m * cap;
-    int cls = S2_CLS_NONE;
-#pragma unroll
-    for (int w = 0; w < 4; ++w) cls = min(cls, point_class(rec[4 * g + w], tab));
-    cls_all[(size_t)m * n_groups + g] = (uint8_t)cls;
 }
 
 // Stable counting sort of the groups by class (positions only), chunk layout, arena layout.

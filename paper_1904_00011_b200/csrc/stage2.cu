@@ -5,12 +5,11 @@
 // Work layout: lanes of a warp are consecutive pixels, every thread owns
 // S2_PX pixels, and the warp walks class-sorted groups of four isochrone points (one Philox call
 // = the four draws of one pixel, R-C1), so every table read is a warp-uniform shared-memory
-// broadcast and every loop is specialised for its class.  The chunks (<= 48 groups of one class)
-// of all (model, 512-pixel tile) pairs form one sequence; it is cut by estimated cost into one
-// contiguous share per persistent CTA (no work queue).  A CTA streams its chunks through a ring of
-// shared-memory stages filled by bulk async copies (TMA) with full/empty mbarriers -- no CTA-wide
-// barrier inside the stream -- and writes one partial flux per (tile fragment, band, pixel);
-// k_reduce_dust adds the (at most a few) fragments of a tile.
+// broadcast and every loop is specialised for its class.  A work unit = (model, 512-pixel tile, segment of the
+// model's chunk list); persistent CTAs take units from an atomic counter, one ahead, and stream the chunks
+// (<= 48 groups of one class) of successive units through a ring of shared-memory stages filled by bulk async
+// copies (TMA) with full/empty mbarriers -- no CTA-wide barrier inside the stream -- and write one partial
+// flux per (unit, band, pixel); k_reduce_dust adds the segments of a tile in a fixed order.
 #include "pcmd_internal.cuh"
 
 #ifndef S2_THREADS
