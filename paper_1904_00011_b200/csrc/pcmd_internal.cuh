@@ -21,17 +21,19 @@ struct __align__(16) PointRec {
 // is cut by estimated cost into n_seg segments, and a work unit = (model, 512-pixel tile, segment).
 // Persistent CTAs take units from an atomic counter (units are fixed, so results do not depend on which
 // CTA ran them) and stream their chunks through a shared-memory ring.
-#define S2_NCLASS 10       // classes, most expensive first:
+#define S2_NCLASS 12       // classes, most expensive first:
 #define S2_CLS_D9 1        //   0 bisection in global memory (tables longer than 511)
-#define S2_CLS_D7 2        //   1-3 branch-free search of a padded table of 2^D words in shared memory
-#define S2_CLS_D5 3
-#define S2_CLS_S4 4        //   4-5 the same search over the first 2^D - 1 thresholds only (k0 = 0 and more stars than that
-#define S2_CLS_S3 5        //       have probability < 2^-10: the overflow path finishes them)
-#define S2_CLS_L4 6        //   6-8 L inline thresholds decide the draw (more stars: probability < 2^-10)
-#define S2_CLS_L2 7
-#define S2_CLS_L1 8
-#define S2_CLS_L0 9        //   9 rare: P(any star) < 2^-8 per draw: one max-compare per group, then class L1's path
-#define S2_CLS_NONE 10     //   no point of the group can have a star: dropped
+#define S2_CLS_D8 2        //   1-5 branch-free search of a padded table of 2^D words in shared memory
+#define S2_CLS_D7 3
+#define S2_CLS_D6 4
+#define S2_CLS_D5 5
+#define S2_CLS_S4 6        //   6-7 the same search over the first 2^D - 1 thresholds only (k0 = 0 and more stars than that
+#define S2_CLS_S3 7        //       have probability < 2^-10: the overflow path finishes them)
+#define S2_CLS_L4 8        //   8-10 L inline thresholds decide the draw (more stars: probability < 2^-10)
+#define S2_CLS_L2 9
+#define S2_CLS_L1 10
+#define S2_CLS_L0 11       //   11 rare: P(any star) < 2^-8 per draw: one max-compare per group, then class L1's path
+#define S2_CLS_NONE 12     //   no point of the group can have a star: dropped
 #define S2_CHUNK 48         // group records per staged chunk (48 * 160 B = 7.5 KB)
 #ifndef S2_TABW
 #define S2_TABW 4096        // words of staged search tables per chunk (16 KB): 32 / 8 / 2 groups of D5 / D7 / D9
@@ -39,7 +41,9 @@ struct __align__(16) PointRec {
 // cost model of the segment cut: ~SM cycles per warp and group of each class loop (profiles/), and per chunk
 #define S2_COST_G 1500u
 #define S2_COST_D9 420u
+#define S2_COST_D8 390u
 #define S2_COST_D7 340u
+#define S2_COST_D6 295u
 #define S2_COST_D5 250u
 #define S2_COST_S4 225u
 #define S2_COST_S3 205u
@@ -50,7 +54,8 @@ struct __align__(16) PointRec {
 #define S2_COST_CHUNK 100u
 // log2 of the padded table size of a search class
 __host__ __device__ __forceinline__ int s2_class_depth(int cls) {
-    return cls == S2_CLS_D9 ? 9 : (cls == S2_CLS_D7 ? 7 : (cls == S2_CLS_D5 ? 5 : (cls == S2_CLS_S4 ? 4 : (cls == S2_CLS_S3 ? 3 : 0))));
+    return cls == S2_CLS_D9 ? 9 : cls == S2_CLS_D8 ? 8 : cls == S2_CLS_D7 ? 7 : cls == S2_CLS_D6 ? 6 : cls == S2_CLS_D5 ? 5
+           : cls == S2_CLS_S4 ? 4 : cls == S2_CLS_S3 ? 3 : 0;
 }
 struct __align__(16) GroupRec {      // 160 bytes
     uint32_t g_orig, cls, tmin, pad1; // original group index (Philox counter word 1), class, min over w of T[0][w]

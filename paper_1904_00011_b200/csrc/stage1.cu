@@ -228,7 +228,9 @@ __device__ __forceinline__ int point_class(const PointRec &r, const uint32_t *__
         if (r.len <= 15 || tab[r.off + 15] >= S2_OVF_THR) return S2_CLS_S4;
     }
     if (r.len <= 31) return S2_CLS_D5;
+    if (r.len <= 63) return S2_CLS_D6;
     if (r.len <= 127) return S2_CLS_D7;
+    if (r.len <= 255) return S2_CLS_D8;
     if (r.len <= 511) return S2_CLS_D9;
     return 0;
 }
@@ -238,7 +240,7 @@ __device__ __forceinline__ int point_class(const PointRec &r, const uint32_t *__
 //
 // Cost model of stage 2 (cost units ~ SM cycles per warp and group, measured per class loop with
 // ncu, profiles/): the static partition of the chunk sequence among the persistent CTAs is by cost.
-__constant__ uint32_t c_s2_group_cost[S2_NCLASS] = {S2_COST_G, S2_COST_D9, S2_COST_D7, S2_COST_D5, S2_COST_S4, S2_COST_S3,
+__constant__ uint32_t c_s2_group_cost[S2_NCLASS] = {S2_COST_G, S2_COST_D9, S2_COST_D8, S2_COST_D7, S2_COST_D6, S2_COST_D5, S2_COST_S4, S2_COST_S3,
                                                     S2_COST_L4, S2_COST_L2, S2_COST_L1, S2_COST_L0};
 __global__ void __launch_bounds__(1024) k_group_sort(const uint8_t *__restrict__ cls_all, int Jpad,
                                                      int64_t arena_cap, uint32_t *__restrict__ pos_all,
@@ -284,7 +286,7 @@ __global__ void __launch_bounds__(1024) k_group_sort(const uint8_t *__restrict__
         ModelPlan t;
         // padded search tables: D9 first, then D7, D5; a class that does not fit the arena is
         // demoted to bisection in global memory (run_cls = 0)
-        const int64_t stride[6] = {0, 4 << 9, 4 << 7, 4 << 5, 4 << 4, 4 << 3};      // words of padded tables per group
+        const int64_t stride[8] = {0, 4 << 9, 4 << 8, 4 << 7, 4 << 6, 4 << 5, 4 << 4, 4 << 3};      // words of padded tables per group
         int first_d = S2_CLS_D9;
         for (;;) {
             int64_t need = 0;

@@ -533,7 +533,9 @@ __global__ void __launch_bounds__(S2_THREADS, S2_MINB) k_stage2(const S2Args a) 
         else if (d.cls == S2_CLS_S3) { S2_LOOP((group_search<NB, COUNTS, 3, true>(st, gr, u, xs + ((uint32_t)g << 7), cx, rec, tab, a.mult))) }
         else if (d.cls == S2_CLS_S4) { S2_LOOP((group_search<NB, COUNTS, 4, true>(st, gr, u, xs + ((uint32_t)g << 8), cx, rec, tab, a.mult))) }
         else if (d.cls == S2_CLS_D5) { S2_LOOP((group_search<NB, COUNTS, 5, false>(st, gr, u, xs + ((uint32_t)g << 9), cx, rec, tab, a.mult))) }
+        else if (d.cls == S2_CLS_D6) { S2_LOOP((group_search<NB, COUNTS, 6, false>(st, gr, u, xs + ((uint32_t)g << 10), cx, rec, tab, a.mult))) }
         else if (d.cls == S2_CLS_D7) { S2_LOOP((group_search<NB, COUNTS, 7, false>(st, gr, u, xs + ((uint32_t)g << 11), cx, rec, tab, a.mult))) }
+        else if (d.cls == S2_CLS_D8) { S2_LOOP((group_search<NB, COUNTS, 8, false>(st, gr, u, xs + ((uint32_t)g << 12), cx, rec, tab, a.mult))) }
         else if (d.cls == S2_CLS_D9) { S2_LOOP((group_search<NB, COUNTS, 9, false>(st, gr, u, xs + ((uint32_t)g << 13), cx, rec, tab, a.mult))) }
         else { S2_LOOP((group_generic<NB, COUNTS>(st, gr, u, rec, tab, a.mult))) }
 #undef S2_LOOP
