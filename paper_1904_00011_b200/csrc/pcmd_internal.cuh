@@ -36,7 +36,7 @@ struct __align__(16) PointRec {
 #define S2_CLS_NONE 12     //   no point of the group can have a star: dropped
 #define S2_CHUNK 48         // group records per staged chunk (48 * 160 B = 7.5 KB)
 #ifndef S2_TABW
-#define S2_TABW 4096        // words of staged search tables per chunk (16 KB): 32 / 8 / 2 groups of D5 / D7 / D9
+#define S2_TABW 6144        // words of staged search tables per chunk (24 KB): 48 / 24 / 12 / 6 / 3 groups of D5 / D6 / D7 / D8 / D9
 #endif
 // cost model of the segment cut: ~SM cycles per warp and group of each class loop (profiles/), and per chunk
 #define S2_COST_G 1500u
@@ -285,6 +285,33 @@ __device__ __forceinline__ uint32_t count_below(const uint32_t *__restrict__ T, 
         if (u > T[mid]) lo = mid + 1; else hi = mid;
     }
     return lo;
+}
+
+// bulk async copy (TMA, UBLKCP in SASS) + mbarrier helpers shared by stage 2 and the convolution ------------
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t *bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t *bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_LOOP_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra WAIT_DONE_%=;\n"
+        "bra WAIT_LOOP_%=;\n"
+        "WAIT_DONE_%=:\n"
+        "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void *dst, const void *src, uint32_t bytes, uint64_t *bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
 }
 
 // launchers implemented in the stage files ---------------------------------------------------

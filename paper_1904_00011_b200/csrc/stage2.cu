@@ -49,14 +49,7 @@ struct S2Args {
     uint32_t *total;         // optional [n_models][P], zeroed before the launch
 };
 
-// ---- bulk async copy (TMA) + mbarrier ---------------------------------------------------------
-__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void mbar_init(uint64_t *bar, uint32_t count) {
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
-}
-__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes) {
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
-}
+// ---- bulk async copy (TMA) + mbarrier: the plain forms are in pcmd_internal.cuh ------------------
 // lane-predicated forms for the warp-uniform producer
 __device__ __forceinline__ void mbar_expect_tx_if(bool lead, uint64_t *bar, uint32_t bytes) {
     asm volatile("{\n.reg .pred q;\nsetp.ne.b32 q, %2, 0;\n@q mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n}"
@@ -70,24 +63,6 @@ __device__ __forceinline__ void bulk_g2s_if(bool lead, void *dst, const void *sr
     asm volatile("{\n.reg .pred q;\nsetp.ne.b32 q, %4, 0;\n"
                  "@q cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];\n}"
                  ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)), "r"((int)lead) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive(uint64_t *bar) {
-    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity) {
-    asm volatile(
-        "{\n"
-        ".reg .pred p;\n"
-        "WAIT_LOOP_%=:\n"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
-        "@p bra WAIT_DONE_%=;\n"
-        "bra WAIT_LOOP_%=;\n"
-        "WAIT_DONE_%=:\n"
-        "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
-}
-__device__ __forceinline__ void bulk_g2s(void *dst, const void *src, uint32_t bytes, uint64_t *bar) {
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
-                 ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
 }
 // Stores of the producer thread into shared memory.  They go through inline PTX on purpose: a plain C++
 // store to shared memory inside the chunk loop makes the compiler give up warp-uniformity of everything
