@@ -311,19 +311,22 @@ __global__ void __launch_bounds__(C2_THREADS, (NOISE ? 4 : C2_MINB_CLEAN)) k_con
     if (VEC) {
         constexpr int NQ = SW / 4;                 // 16-byte segments per halo row (18 ... 22)
         // N % 4 == 0: a segment never straddles the edge.  Flat index over (row, segment): every lane copies.
-        if (big) {      // (row, segment) and the wrapped source row advance incrementally: no division, no modulo
-            constexpr int DI = C2_THREADS / NQ, DQ = C2_THREADS - DI * NQ;
-            const int i0 = tid / NQ;
-            int q = tid - i0 * NQ, gx4 = x0 - RA + 4 * q, gy = y0 - R + i0;
-            gy += gy < 0 ? N : 0; gy -= gy >= N ? N : 0;
-            uint32_t dst = (uint32_t)__cvta_generic_to_shared(reinterpret_cast<float4 *>(tile) + tid);
-            for (int t = tid; t < rows_used * NQ; t += C2_THREADS) {
-                int gx = gx4;
+        if (big) {      // a thread keeps its 16-byte column segment and walks down the rows: only the wrapped source row changes
+            constexpr int RPI = C2_THREADS / NQ;                  // rows per sweep of the CTA (11 ... 14)
+            if (tid < RPI * NQ) {
+                const int r0 = tid / NQ, q = tid - r0 * NQ;
+                int gx = x0 - RA + 4 * q, gy = y0 - R + r0;
                 gx += gx < 0 ? N : 0; gx -= gx >= N ? N : 0;
-                asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(F + ((size_t)(uint32_t)(gy * N + gx))) : "memory");
-                dst += C2_THREADS * 16; q += DQ; gx4 += 4 * DQ; gy += DI;
-                if (q >= NQ) { q -= NQ; gx4 -= 4 * NQ; gy += 1; }
-                gy -= gy >= N ? N : 0;
+                gy += gy < 0 ? N : 0; gy -= gy >= N ? N : 0;
+                const float *src = F + gx;
+                uint32_t dst = (uint32_t)__cvta_generic_to_shared(reinterpret_cast<float4 *>(tile) + tid);
+#pragma unroll
+                for (int it = 0; it < (SH + RPI - 1) / RPI; ++it) {
+                    if (r0 + it * RPI < rows_used)
+                        asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src + (uint32_t)(gy * N)) : "memory");
+                    gy += RPI; gy -= gy >= N ? N : 0;
+                    dst += RPI * NQ * 16;
+                }
             }
         } else {
             for (int t = tid; t < rows_used * NQ; t += C2_THREADS) {
