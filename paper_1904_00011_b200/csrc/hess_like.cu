@@ -35,10 +35,12 @@ __global__ void __launch_bounds__(HS_THREADS) k_hess(const float *__restrict__ m
     auto one = [&](float a, float b, float y) {
         if (isnan(a) || isnan(b) || isnan(y)) { n_bad++; return; }
         const float x = __fsub_rn(a, b);
-        const float fx = floorf(__fmul_rn(__fsub_rn(x, S.x_lo), S.inv_dx));
-        const float fy = floorf(__fmul_rn(__fsub_rn(y, S.y_lo), S.inv_dy));
-        if (!(fx >= 0.0f) || !(fx < (float)S.nx) || !(fy >= 0.0f) || !(fy < (float)S.ny)) { n_out++; return; }
-        const int bin = (int)fy * S.nx + (int)fx;
+        // floor and conversion in one instruction (saturating, so a far-out value stays out); 0 <= ix < nx as one
+        // unsigned compare: the same decision as floorf + float range test
+        const int ix = __float2int_rd(__fmul_rn(__fsub_rn(x, S.x_lo), S.inv_dx));
+        const int iy = __float2int_rd(__fmul_rn(__fsub_rn(y, S.y_lo), S.inv_dy));
+        if ((unsigned)ix >= (unsigned)S.nx || (unsigned)iy >= (unsigned)S.ny) { n_out++; return; }
+        const int bin = iy * S.nx + ix;
         if (SMEM) atomicAdd(&sh[bin], 1u); else atomicAdd(&gh[bin], 1u);
         n_in++; sx += (double)x; sy += (double)y;
     };
