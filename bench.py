@@ -50,7 +50,7 @@ PHILOX_TEST = "Philox4x32-10 call"
 # dram__bytes_read.sum + dram__bytes_write.sum of one k_stage2 launch from the committed captures: c3 and c5 from
 # `ncu --set full` (profiles/r2_stage2.md), c4 x 64 models from the `--metrics` launch list (profiles/r2_launches.md);
 # None for configurations / batches that were not captured
-NCU_TRAFFIC_BYTES = {("c3", 1): 1.323e6 + 0.195e6, ("c5", 1): 12.376e6 + 0.042e6, ("c4", 64): 40.84e6 + 2.91e6}
+NCU_TRAFFIC_BYTES = {("c3", 1): 1.273e6 + 0.144e6, ("c5", 1): 8.408e6 + 0.102e6, ("c4", 64): 41.04e6 + 3.06e6}
 
 
 def i_alg(n_bands: int) -> int:

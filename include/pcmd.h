@@ -110,7 +110,11 @@ void pcmd_destroy(pcmd_ctx *ctx);
  *   d_flux_raw    DEVICE out, same shape, stage-2 flux in electrons; may be NULL
  *   d_count_hash  DEVICE out [n_models][P] uint64, sum_j n_pj*(splitmix64(j)|1) mod 2^64;
  *   d_count_total DEVICE out [n_models][P] uint32, sum_j n_pj.  Both NULL (production) or both
- *                 non-NULL (parity build of the same kernel, which also tracks integer counts). */
+ *                 non-NULL (parity build of the same kernel, which also tracks integer counts).
+ * With cfg.sampler_mode = 1 the star counts come from the aggregated sampler (R-A1); every output keeps
+ * its meaning.  Errors: PCMD_EINVAL (NULL / non-finite / negative parameters, sigma <= 0), PCMD_ERANGE (an
+ * expected count above 2^22; raised on the host when it can be seen there, else by the device: pcmd_status),
+ * PCMD_ENOMEM, PCMD_ECUDA. */
 int  pcmd_simulate(pcmd_ctx *ctx, const pcmd_params *params, int32_t n_models,
                    uint64_t seed, uint32_t model_index0,
                    float *d_mag, float *d_flux_raw,
