@@ -173,3 +173,15 @@ def test_capped_arena_non_power_of_two_batch():
         assert np.array_equal(r["total"][i], o["total"]) and np.array_equal(r["hash"][i], o["hash"])
         assert np.allclose(r["raw"][i], o["F_raw"], rtol=1e-5, atol=0)
     r["g"].close()
+
+
+def test_pipe_bench_reports_sane_rates():
+    """pcmd_pipe_bench (measurement support, csrc/pipes.cu): every stream runs and reports a rate between 0 and 2
+    warp-instructions per clock per scheduler; the Philox-only kernel lands between 1e12 and 2.4e12 draws/s on a B200."""
+    G = _G()
+    rows = G.pipe_bench(iters=512)
+    assert len(rows) >= 10 and all(0.0 < r["rate"] < 2.0 and r["ms"] > 0 for r in rows)
+    ph = [r for r in rows if r["name"].startswith("Philox4x32-10")][0]
+    assert 1.0e12 < 4.0 * ph["steps_per_s"] < 2.4e12
+    one = G.pipe_bench(iters=512, only="LOP3 (xor3)")
+    assert len(one) == 1 and 0.4 < one[0]["rate"] < 0.6
