@@ -34,7 +34,9 @@ struct __align__(16) PointRec {
 #define S2_CLS_L1 10
 #define S2_CLS_L0 11       //   11 rare: P(any star) < 2^-8 per draw: one max-compare per group, then class L1's path
 #define S2_CLS_NONE 12     //   no point of the group can have a star: dropped
+#ifndef S2_CHUNK
 #define S2_CHUNK 48         // group records per staged chunk (48 * 160 B = 7.5 KB)
+#endif
 #ifndef S2_TABW
 #define S2_TABW 6144        // words of staged search tables per chunk (24 KB): 48 / 24 / 12 / 6 / 3 groups of D5 / D6 / D7 / D8 / D9
 #endif
