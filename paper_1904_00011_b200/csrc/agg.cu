@@ -133,6 +133,8 @@ __global__ void __launch_bounds__(AGG_THREADS) k_stage2_agg(const AggArgs a) {
         const uint64_t r0 = __umul64hi(((uint64_t)w[0] << 32) | w[1], W), r1 = __umul64hi(((uint64_t)w[2] << 32) | w[3], W);
         int lo0 = (int)G[(uint32_t)(r0 >> AGG_SHIFT)], hi0 = (int)G[(uint32_t)(r0 >> AGG_SHIFT) + 1];
         int lo1 = (int)G[(uint32_t)(r1 >> AGG_SHIFT)], hi1 = (int)G[(uint32_t)(r1 >> AGG_SHIFT) + 1];
+        PCMD_CHK((r0 >> AGG_SHIFT) + 1 < AGG_CELLS && (r1 >> AGG_SHIFT) + 1 < AGG_CELLS && r0 < W && r1 < W);
+        PCMD_CHK(lo0 >= 0 && lo0 <= hi0 && hi0 < a.J && lo1 >= 0 && lo1 <= hi1 && hi1 < a.J);
         while (lo0 < hi0 || lo1 < hi1) {            // the j with C_j <= r < C_{j+1}
             const int m0 = (lo0 + hi0 + 1) >> 1, m1 = (lo1 + hi1 + 1) >> 1;
             const uint64_t c0 = C[m0], c1 = C[m1];
@@ -140,6 +142,7 @@ __global__ void __launch_bounds__(AGG_THREADS) k_stage2_agg(const AggArgs a) {
             if (lo1 < hi1) { if (c1 <= r1) lo1 = m1; else hi1 = m1 - 1; }
         }
         const bool two = s + 1 < N;
+        PCMD_CHK(C[lo0] <= r0 && r0 < C[lo0 + 1] && C[lo1] <= r1 && r1 < C[lo1 + 1]);
         const float4 f0 = *reinterpret_cast<const float4 *>(rec[lo0].f);
         const float4 f1 = two ? *reinterpret_cast<const float4 *>(rec[lo1].f) : make_float4(0.f, 0.f, 0.f, 0.f);
         F[0] += (double)f0.x; F[1] += (double)f0.y; F[2] += (double)f0.z; F[3] += (double)f0.w;

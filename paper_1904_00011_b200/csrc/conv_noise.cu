@@ -294,6 +294,8 @@ __global__ void __launch_bounds__(C2_THREADS, (NOISE ? 4 : C2_MINB_CLEAN)) k_con
     constexpr int SH = C2_TH + K - 1;             // halo-tile rows
     constexpr int NV = (OFF + K + 3 + 3) / 4;     // 16-byte loads of one row-pass window
     constexpr int SKY_CAP = 1024;                 // Poisson-sky thresholds kept in shared memory
+    static_assert((C2_TW / 4 - 1 + NV) * 4 <= SW, "row-pass window leaves the halo row");
+    static_assert(C2_TH - 4 + K + 2 < SH, "column-pass window leaves the halo tile");
     extern __shared__ __align__(16) float sm[];
     float *tile = sm;                             // [SH][SW]
     float *hrow = sm;                             // row results overwrite the first 64 columns of their own tile row (stride SW)
@@ -326,6 +328,7 @@ __global__ void __launch_bounds__(C2_THREADS, (NOISE ? 4 : C2_MINB_CLEAN)) k_con
                 uint32_t dst = (uint32_t)__cvta_generic_to_shared(reinterpret_cast<float4 *>(tile) + tid);
 #pragma unroll
                 for (int it = 0; it < (SH + RPI - 1) / RPI; ++it) {
+                    PCMD_CHK(r0 + it * RPI >= rows_used || (gx >= 0 && gx + 3 < N && gy >= 0 && gy < N && tid + it * RPI * NQ < SH * NQ));
                     if (r0 + it * RPI < rows_used)
                         asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src + (uint32_t)(gy * N)) : "memory");
                     gy += RPI; gy -= gy >= N ? N : 0;
@@ -336,6 +339,7 @@ __global__ void __launch_bounds__(C2_THREADS, (NOISE ? 4 : C2_MINB_CLEAN)) k_con
             for (int t = tid; t < rows_used * NQ; t += C2_THREADS) {
                 const int i = t / NQ, q = t - i * NQ;
                 const int gy = wrap_any(y0 - R + i, N), gx = wrap_any(x0 - RA + 4 * q, N);
+                PCMD_CHK(gx >= 0 && gx + 3 < N && gy >= 0 && gy < N && t < SH * NQ);
                 const uint32_t dst = (uint32_t)__cvta_generic_to_shared(reinterpret_cast<float4 *>(tile) + t);
                 asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(F + (size_t)gy * N + gx) : "memory");
             }
@@ -420,6 +424,7 @@ __global__ void __launch_bounds__(C2_THREADS, (NOISE ? 4 : C2_MINB_CLEAN)) k_con
     const uint32_t p0 = (uint32_t)yt * (uint32_t)N + (uint32_t)x;
     float *mag = a.mag + (size_t)mb * a.P + p0;
     if (VEC && yt + 3 < N) {                        // the whole 4 x 4 block is inside the image, 16-byte stores
+        PCMD_CHK((int64_t)p0 + 3 * (int64_t)N + 3 < a.P);
         if (a.tap_conv) {
 #pragma unroll
             for (int j = 0; j < 4; ++j)

@@ -41,6 +41,7 @@ __global__ void __launch_bounds__(HS_THREADS) k_hess(const float *__restrict__ m
         const int iy = __float2int_rd(__fmul_rn(__fsub_rn(y, S.y_lo), S.inv_dy));
         if ((unsigned)ix >= (unsigned)S.nx || (unsigned)iy >= (unsigned)S.ny) { n_out++; return; }
         const int bin = iy * S.nx + ix;
+        PCMD_CHK(bin >= 0 && bin < nbins);
         if (SMEM) atomicAdd(&sh[bin], 1u); else atomicAdd(&gh[bin], 1u);
         n_in++; sx += (double)x; sy += (double)y;
     };

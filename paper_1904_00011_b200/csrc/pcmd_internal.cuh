@@ -4,6 +4,18 @@
 #include <stdint.h>
 #include "../../include/pcmd.h"
 
+// Self-check build (PCMD_NVCC_EXTRA=-DPCMD_SELFCHECK, profiles/r2_sanitizers.md): device-side assertions on the
+// staged addresses, table ranges, work-unit indices and shared-memory indices of every kernel; a failed
+// assertion ends the launch with cudaErrorAssert (the call returns PCMD_ECUDA) and prints file:line.
+// The product build compiles them away.
+#ifdef PCMD_SELFCHECK
+#undef NDEBUG
+#include <assert.h>
+#define PCMD_CHK(c) assert(c)
+#else
+#define PCMD_CHK(c) ((void)0)
+#endif
+
 #define PCMD_LAMBDA_MAX 4194304.0 /* 2^22, R-C2 */
 
 // Per isochrone point record consumed by stage 2 (32 bytes, one group of 4 points = 128 B).

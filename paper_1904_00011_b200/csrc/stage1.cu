@@ -413,10 +413,12 @@ __global__ void __launch_bounds__(128) k_points(const DevModel *__restrict__ mdl
                 const uint32_t dst = atomicAdd(&alloc[2 * m + 1], stored);    // stored <= n: the compact region cannot overflow if the raw one did not
                 uint32_t *out = tab_all + (size_t)m * cap;
                 uint32_t wr = dst;
+                PCMD_CHK((int64_t)dst + stored <= cap && mode >= k_lo && mode <= k_hi);
                 for (uint32_t i = 0; i < n; ++i) {
                     const unsigned long long t = (unsigned long long)__double_as_longlong(q[i]);
                     if (t != 0ull && t < 4294967296ull) out[wr++] = (uint32_t)(t - 1ull);
                 }
+                PCMD_CHK(wr == dst + stored);
                 r.k0 = (uint32_t)k_lo + zeros; r.len = stored; r.off = dst;
                 r.T0 = stored ? out[dst] : 0xFFFFFFFFu;
                 pcls = point_class(r, out);

@@ -143,6 +143,7 @@ __device__ __forceinline__ void overflow_fixup(S2State<NB, COUNTS> &st, const Gr
         for (int i = 0; i < S2_PX; ++i) {
             if (u[i][w] > Tov) {
                 const PointRec r = rec[j];
+                PCMD_CHK(r.len >= (uint32_t)L + 1u);      // the overflow threshold is entry L of the table
                 const uint32_t extra = 1u + count_below(tab + r.off + L + 1, r.len - (L + 1), u[i][w]);
                 add_stars<NB, COUNTS>(st, i, (float)extra, *reinterpret_cast<const float4 *>(g->f[w]), j, mult);
             }
@@ -292,6 +293,8 @@ __device__ __forceinline__ void group_search(S2State<NB, COUNTS> &st, const Grou
             }
             // off = (address of X[pos]) 2^-149 -> address / 4 + kq = k0 + pos, in two exact steps (2^147 is not a float)
             const float nf = fmaf(off * 8.507059173023462e37f, 2097152.0f, kq[w]);
+            PCMD_CHK(__float_as_uint(off) - base <= (4u << D) - 4u && ((__float_as_uint(off) - base) & 3u) == 0u);
+            PCMD_CHK(nf >= 0.f && nf < 4194304.f && nf == floorf(nf));
             add_stars<NB, COUNTS>(st, i, nf, f, g->g_orig * 4u + w, mult);
         }
     }
@@ -304,6 +307,7 @@ __device__ __forceinline__ void group_search(S2State<NB, COUNTS> &st, const Grou
             for (int i = 0; i < S2_PX; ++i) {
                 if (u[i][w] > tov[w]) {
                     const PointRec r = rec[j];
+                    PCMD_CHK(r.len >= (1u << D));            // the overflow threshold is entry 2^D - 1
                     const uint32_t extra = 1u + count_below(tab + r.off + (1u << D), r.len - (1u << D), u[i][w]);
                     add_stars<NB, COUNTS>(st, i, (float)extra, *reinterpret_cast<const float4 *>(g->f[w]), j, mult);
                 }
@@ -383,6 +387,8 @@ __device__ __forceinline__ void s2_advance(const S2Args &a, S2Shared &sh, bool l
         const int hi = seg + 1 == ns ? p.n_chunks : s2_first_chunk_at(p, (uint32_t)((uint64_t)C * (seg + 1) / ns));
         int cls = 0;
         while (lo >= p.chunk_start[cls + 1]) cls++;
+        PCMD_CHK(m >= 0 && m < a.n_models && tile >= 0 && tile < a.n_tiles && lo >= 0 && lo < hi && hi <= p.n_chunks &&
+                 cls < S2_NCLASS);
         sts128(lead, &sh.m_, make_int4(m, tile, seg, lo));
         sts128(lead, &sh.chunk_end, make_int4(hi, cls, 1, sh.issued));
         __syncwarp();
@@ -403,6 +409,9 @@ __device__ __forceinline__ void s2_issue(const S2Args &a, S2Shared &sh, GroupRec
     const uint32_t rbytes = (uint32_t)ng * (uint32_t)sizeof(GroupRec), tbytes = D ? ((uint32_t)ng << (D + 4)) : 0u;
     const GroupRec *rsrc = a.grp + (size_t)mt * a.n_groups + g0;
     const uint32_t *tsrc = a.arena + (size_t)mt * a.arena_cap + p.arena_off[cls] + ((size_t)(g0 - p.cls_start[cls]) << (D + 2));
+    PCMD_CHK(cls >= 0 && cls < S2_NCLASS && li >= 0 && ng >= 1 && ng <= S2_CHUNK && g0 >= 0 && g0 + ng <= a.n_groups);
+    PCMD_CHK(tbytes <= (uint32_t)S2_TABW * 4u && (rbytes & 15u) == 0u && s >= 0 && s < S2_NST);
+    PCMD_CHK(!D || (size_t)p.arena_off[cls] + ((size_t)(g0 - p.cls_start[cls] + ng) << (D + 2)) <= (size_t)a.arena_cap);
     ChunkDesc d;
     d.m = m; d.tile = sh.tile; d.cls = run; d.ng = ng; d.slot = sh.seg; d.pad0 = d.pad1 = 0;
     // step: next chunk of the unit, or the next unit (which may replace sh.plan: everything above is in locals)
@@ -467,6 +476,8 @@ __global__ void __launch_bounds__(S2_THREADS, S2_MINB) k_stage2(const S2Args a) 
         mbar_wait(&sh.full[s], par);
         const ChunkDesc d = sh.desc[s];
         const int mt = d.m * a.mts;
+        PCMD_CHK(d.m >= 0 && d.m < a.n_models && d.tile >= 0 && d.tile < a.n_tiles && d.slot >= 0 && d.slot < a.n_seg &&
+                 d.ng >= 0 && d.ng <= S2_CHUNK && d.cls >= 0 && d.cls <= S2_NCLASS);
         if (d.flags & S2_F_FIRST) {
             mctr = a.model0 + (uint32_t)d.m;
 #pragma unroll
