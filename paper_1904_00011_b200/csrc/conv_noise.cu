@@ -233,17 +233,15 @@ __device__ __forceinline__ int wrap_any(int v, int N) {
     return v < 0 ? v + N : v;
 }
 
-// zp - 2.5 log10(arg) for arg > 0: exponent by the add-magic-constant trick (no int->float conversion),
-// mantissa by the special-function unit, finished in fp32 with split constants
+// zp - 2.5 log10(arg) for arg > 0: one lg2.approx on the special-function unit (it handles the exponent itself: no
+// exponent / mantissa split, no denormal pre-scaling of __log2f), finished in fp32 with split constants
 __device__ __forceinline__ float mag_of(float arg, double zp) {
     // branch-free: the 16 magnitudes of a thread are independent chains the scheduler can interleave
-    const uint32_t bits = __float_as_uint(fmaxf(arg, 1.17549435e-38f));
-    const float e = __uint_as_float(0x4B000000u | (bits >> 23)) - 8388735.0f;      // (2^23 + biased exponent) - 2^23 - 127
-    const float mant = __uint_as_float((bits & 0x007FFFFFu) | 0x3F800000u);
     // zp and -2.5 log10(2) as float pairs: two fp32 FMAs instead of float->double, fp64 FMA, double->float (the conversion
-    // unit is a scarce pipe here).  Measured against the oracle's stage 5: max 2.3e-6 mag (fp64 finish: 1.6e-6).
+    // unit is a scarce pipe here).  Measured against the oracle's stage 5: max 1.7e-6 mag (fp64 finish: 1.6e-6).
     const float zph = (float)zp, zpl = (float)(zp - (double)zph);
-    const float l2 = e + __log2f(mant);
+    float l2;
+    asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(l2) : "f"(fmaxf(arg, 1.17549435e-38f)));   // a denormal flux is not flushed to -inf
     const float mg = fmaf(l2, -0.752574980258941650390625f, zph) + fmaf(l2, -8.901011e-9f, zpl);
     return arg > 0.f ? mg : __int_as_float(0x7fc00000);
 }
