@@ -29,6 +29,7 @@ extern "C" {
 #define PCMD_ERANGE  -2   /* an expected star count lambda_j exceeds 2^22 (R-C2)               */
 #define PCMD_ENOMEM  -3   /* host or device allocation failed                                  */
 #define PCMD_ECUDA   -4   /* a CUDA call failed; pcmd_last_cuda_error(ctx) gives the code      */
+#define PCMD_ELIMIT  -5   /* the request exceeds the fixed scratch of a no-allocation entry point */
 
 #define PCMD_MAX_BANDS 4
 #define PCMD_MAX_HESS  4
@@ -135,6 +136,28 @@ int  pcmd_simulate_repeat(pcmd_ctx *ctx, const pcmd_params *params, int32_t n_re
  *   d_stats  DEVICE out [n_models][n_hess]; may be NULL */
 int  pcmd_hess(pcmd_ctx *ctx, const float *d_mag, int32_t n_models,
                uint32_t *d_hess, pcmd_hess_stats *d_stats, void *cuda_stream);
+
+/* Stage 6 for callers that must not allocate (code under CUDA graph capture, tight serving loops,
+ * harnesses that forbid cudaMalloc): the same kernels, launch geometry, arguments and results as
+ * pcmd_hess (bit-identical diagrams and statistics), but the per-block partial statistics go to a
+ * fixed array in the library's device image instead of the ctx's grow-on-demand scratch.  The call
+ * makes no cudaMalloc / cudaFree / allocating library call.
+ *   limit   n_models * n_hess * (blocks per diagram) <= PCMD_HESS_NOALLOC_MAX_PARTS (32 bytes each:
+ *           256 KB that every GPU which loads the library holds until exit); a larger request returns
+ *           PCMD_ELIMIT and launches nothing.  pcmd_hess_noalloc_parts(ctx, n_models) returns the
+ *           number a call would need (blocks per diagram = 1 once n_models * n_hess >= 8 * SMs).
+ *   sharing the array is ONE per device and process, shared by every ctx and every call; it keeps the
+ *           last call's contents (nothing in it has to start at zero: every slot a call reads it has
+ *           written first).  Two calls that overlap on the GPU (different streams, or graphs replayed
+ *           concurrently) race on it: serialise them.
+ *   set-up  the array's device address is looked up once per device on the first call, or by
+ *           pcmd_hess_noalloc_setup() (no arguments: the CURRENT device) -- call that before starting
+ *           a graph capture.  Returns PCMD_OK or PCMD_ECUDA. */
+#define PCMD_HESS_NOALLOC_MAX_PARTS 8192
+int     pcmd_hess_noalloc_setup(void);
+int64_t pcmd_hess_noalloc_parts(const pcmd_ctx *ctx, int32_t n_models);
+int     pcmd_hess_noalloc(pcmd_ctx *ctx, const float *d_mag, int32_t n_models,
+                          uint32_t *d_hess, pcmd_hess_stats *d_stats, void *cuda_stream);
 
 /* Stage 7: log-likelihood of the data Hess given each model Hess, summed over the n_hess
  * diagrams.  like_mode: PCMD_LIKE_*.  d_stats / d_data_stats are needed by the GAUSS modes

@@ -79,6 +79,10 @@ def lib():
         L.pcmd_simulate.argtypes = [vp, vp, i32, u64, u32, vp, vp, vp, vp, vp]
         L.pcmd_simulate_repeat.argtypes = [vp, vp, i32, u64, u32, vp, vp, vp, vp, vp]
         L.pcmd_hess.argtypes = [vp, vp, i32, vp, vp, vp]
+        L.pcmd_hess_noalloc.argtypes = [vp, vp, i32, vp, vp, vp]
+        L.pcmd_hess_noalloc_setup.argtypes = []
+        L.pcmd_hess_noalloc_parts.argtypes = [vp, i32]
+        L.pcmd_hess_noalloc_parts.restype = i64
         L.pcmd_loglike.argtypes = [vp, vp, vp, i32, vp, vp, i32, vp, vp]
         L.pcmd_evaluate_host.argtypes = [vp, vp, i32, u64, u32, vp, vp, i32, vp, vp, vp, vp]
         L.pcmd_hess_bins_total.argtypes = [vp]
@@ -280,6 +284,17 @@ class Pcmd:
         if rc:
             raise PcmdError(rc, "pcmd_hess")
         return H, st
+
+    def hess_noalloc(self, mag, out, stats=None):
+        """pcmd_hess_noalloc: stage 6 into the caller's `out` (and `stats`), no allocation anywhere on the way
+        (include/pcmd.h: fixed scratch of PCMD_HESS_NOALLOC_MAX_PARTS partials, shared per device)."""
+        rc = lib().pcmd_hess_noalloc(self._ctx, _dp(mag), mag.shape[0], _dp(out), _dp(stats), self._stream())
+        if rc:
+            raise PcmdError(rc, "pcmd_hess_noalloc")
+        return out, stats
+
+    def hess_noalloc_parts(self, n_models):
+        return int(lib().pcmd_hess_noalloc_parts(self._ctx, int(n_models)))
 
     def loglike(self, H, stats, data_hess, data_stats=None, mode=LIKE_POISSON):
         t = self.torch

@@ -28,6 +28,7 @@ extern "C" const char *pcmd_strerror(int code) {
         case PCMD_ERANGE: return "expected star count of an isochrone point exceeds 2^22";
         case PCMD_ENOMEM: return "out of memory";
         case PCMD_ECUDA: return "CUDA error";
+        case PCMD_ELIMIT: return "request exceeds the fixed scratch of a no-allocation entry point";
         default: return "unknown error";
     }
 }

@@ -266,3 +266,89 @@ int pcmd_launch_loglike(pcmd_ctx *c, const uint32_t *d_hm, const pcmd_hess_stats
     PCMD_LAUNCHED(c);
     return PCMD_OK;
 }
+
+// ---------------------------------------------------------------------------------------------
+// pcmd_hess_noalloc (include/pcmd.h): stage 6 without any allocation.  The per-block partial statistics of
+// k_hess go to a fixed array in this module's device image (one per device that loads the library, held
+// until exit) instead of ctx->d_hpart.  Same kernels, same launch geometry as pcmd_launch_hess: results
+// are bit-identical.  Nothing in the array has to start at zero (k_hess writes every slot k_hess_stats
+// reads); it is shared by every call on the device, so calls that overlap on the GPU race on it.
+static __device__ __align__(256) pcmd_hess_stats g_hess_parts[PCMD_HESS_NOALLOC_MAX_PARTS];
+
+#define HS_MAX_DEVICES 64
+// In host code `g_hess_parts` is only a handle for the runtime's symbol table, not a device address: the
+// address is looked up per device (with that device current) and cached here.
+static pcmd_hess_stats *g_hess_parts_addr[HS_MAX_DEVICES];
+
+static cudaError_t hess_noalloc_addr(pcmd_hess_stats **out) {
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= HS_MAX_DEVICES) return cudaErrorInvalidDevice;
+    pcmd_hess_stats *p = __atomic_load_n(&g_hess_parts_addr[dev], __ATOMIC_ACQUIRE);
+    if (!p) {
+        e = cudaGetSymbolAddress((void **)&p, g_hess_parts);
+        if (e != cudaSuccess) return e;
+        if (!p) return cudaErrorInvalidSymbol;
+        __atomic_store_n(&g_hess_parts_addr[dev], p, __ATOMIC_RELEASE);   // every thread looks up the same address
+    }
+    *out = p;
+    return cudaSuccess;
+}
+
+extern "C" int pcmd_hess_noalloc_setup(void) {
+    pcmd_hess_stats *p = nullptr;
+    return hess_noalloc_addr(&p) == cudaSuccess ? PCMD_OK : PCMD_ECUDA;
+}
+
+// blocks per diagram and pixels per block: the rule of pcmd_launch_hess
+static int hess_geometry(const pcmd_ctx *c, int n_models, int64_t *ppb_out) {
+    int64_t want_blocks = ((int64_t)c->sm_count * 8) / ((int64_t)n_models * c->n_hess);
+    if (want_blocks < 1) want_blocks = 1;
+    int64_t ppb = (c->P + want_blocks - 1) / want_blocks;
+    if (ppb < HS_PIX_PER_BLOCK) ppb = HS_PIX_PER_BLOCK;
+    ppb = (ppb + 1023) & ~(int64_t)1023;
+    if (ppb_out) *ppb_out = ppb;
+    return (int)((c->P + ppb - 1) / ppb);
+}
+
+extern "C" int64_t pcmd_hess_noalloc_parts(const pcmd_ctx *c, int32_t n_models) {
+    if (!c || n_models < 1 || c->n_hess < 1) return 0;
+    return (int64_t)n_models * c->n_hess * hess_geometry(c, n_models, nullptr);
+}
+
+extern "C" int pcmd_hess_noalloc(pcmd_ctx *c, const float *d_mag, int32_t n_models, uint32_t *d_hess,
+                                 pcmd_hess_stats *d_stats, void *cuda_stream) {
+    if (!c || !d_mag || !d_hess || n_models < 1 || c->n_hess < 1) return PCMD_EINVAL;
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    int64_t ppb = 0;
+    const int nblk = hess_geometry(c, n_models, &ppb);
+    if ((int64_t)n_models * c->n_hess * nblk > PCMD_HESS_NOALLOC_MAX_PARTS) return PCMD_ELIMIT;
+    pcmd_hess_stats *parts = nullptr;
+    PCMD_CUDA(c, hess_noalloc_addr(&parts));
+    int maxbins = 0;
+    for (int h = 0; h < c->n_hess; ++h) maxbins = max(maxbins, c->hess[h].nx * c->hess[h].ny);
+    const size_t smem = (size_t)maxbins * sizeof(uint32_t);
+    PCMD_PROF(c, 4, s);
+    if (!(nblk == 1 && smem <= 200 * 1024))
+        PCMD_CUDA(c, cudaMemsetAsync(d_hess, 0, (size_t)n_models * c->hess_bins * sizeof(uint32_t), s));
+    dim3 grid(nblk, c->n_hess, n_models);
+    if (smem <= 200 * 1024) {
+        if (smem > 48 * 1024 && smem > c->smem_hess) {      // an attribute of the function, not an allocation
+            PCMD_CUDA(c, cudaFuncSetAttribute(k_hess<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+            c->smem_hess = smem;
+        }
+        k_hess<true><<<grid, HS_THREADS, smem, s>>>(d_mag, c->B, c->P, c->d_hess_spec, c->n_hess, ppb,
+                                                    c->hess_bins, d_hess, parts, d_stats);
+    } else {
+        k_hess<false><<<grid, HS_THREADS, 0, s>>>(d_mag, c->B, c->P, c->d_hess_spec, c->n_hess, ppb,
+                                                  c->hess_bins, d_hess, parts, d_stats);
+    }
+    PCMD_LAUNCHED(c);
+    if (d_stats && nblk > 1) {
+        k_hess_stats<<<n_models * c->n_hess, 32, 0, s>>>(parts, nblk, d_stats);
+        PCMD_LAUNCHED(c);
+    }
+    PCMD_PROF(c, 5, s);
+    return PCMD_OK;
+}
