@@ -192,7 +192,7 @@ __device__ __forceinline__ void noise_mag_epilogue(const CvArgs &a, const float 
 #define C2_THREADS 256
 #define C2_KMAX 21
 #ifndef C2_MINB_CLEAN
-#define C2_MINB_CLEAN 5       // CTAs per SM of the noise-free instances (register cap 51)
+#define C2_MINB_CLEAN 6       // CTAs per SM of the noise-free instances (register cap 40, no spills; 5 -> 6: K = 7 +3 %, K = 15 flat)
 #endif
 
 struct Cv2Args {
@@ -322,14 +322,21 @@ __global__ void __launch_bounds__(C2_THREADS, (NOISE ? 4 : C2_MINB_CLEAN)) k_con
                 int gx = x0 - RA + 4 * q, gy = y0 - R + r0;
                 gx += gx < 0 ? N : 0; gx -= gx >= N ? N : 0;
                 gy += gy < 0 ? N : 0; gy -= gy >= N ? N : 0;
-                const float *src = F + gx;
+                // byte offset of the wrapped source row, stepped by RPI rows (one conditional subtract wraps it):
+                // 32-bit arithmetic and one 64-bit add per copy; the column's base address is pinned in a register
+                // pair (the compiler otherwise recomputes the whole 64-bit chain under every copy's predicate)
+                unsigned long long src = reinterpret_cast<unsigned long long>(F + gx);
+                asm volatile("" : "+l"(src));
+                const uint32_t NN = (uint32_t)N * (uint32_t)N * 4u, step = (uint32_t)(RPI * N) * 4u;
+                uint32_t off = (uint32_t)gy * (uint32_t)N * 4u;
                 uint32_t dst = (uint32_t)__cvta_generic_to_shared(reinterpret_cast<float4 *>(tile) + tid);
+                const int rem = rows_used - r0;
 #pragma unroll
                 for (int it = 0; it < (SH + RPI - 1) / RPI; ++it) {
-                    PCMD_CHK(r0 + it * RPI >= rows_used || (gx >= 0 && gx + 3 < N && gy >= 0 && gy < N && tid + it * RPI * NQ < SH * NQ));
-                    if (r0 + it * RPI < rows_used)
-                        asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src + (uint32_t)(gy * N)) : "memory");
-                    gy += RPI; gy -= gy >= N ? N : 0;
+                    PCMD_CHK(it * RPI >= rem || (gx >= 0 && gx + 3 < N && off < NN && off % (4u * (uint32_t)N) == 0u && tid + it * RPI * NQ < SH * NQ));
+                    if (it * RPI < rem)
+                        asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src + off) : "memory");
+                    off += step; off -= off >= NN ? NN : 0u;
                     dst += RPI * NQ * 16;
                 }
             }
