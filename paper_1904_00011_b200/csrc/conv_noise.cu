@@ -233,17 +233,18 @@ __device__ __forceinline__ int wrap_any(int v, int N) {
     return v < 0 ? v + N : v;
 }
 
-// zp - 2.5 log10(arg) for arg > 0: one lg2.approx on the special-function unit (it handles the exponent itself: no
-// exponent / mantissa split, no denormal pre-scaling of __log2f), finished in fp32 with split constants
+// zp - 2.5 log10(arg) for arg > 0, NaN for arg <= 0: one lg2.approx on the special-function unit (it handles the
+// exponent itself: no exponent / mantissa split, no denormal pre-scaling of __log2f), finished in fp32 with zp and
+// -2.5 log10(2) as float pairs: two fp32 FMAs instead of float->double, fp64 FMA, double->float (the conversion unit is
+// a scarce pipe here).  The split of -2.5 log10(2) is chosen with a NEGATIVE high part and a POSITIVE low part, so that
+// arg = 0 (lg2 = -inf) gives (+inf) + (-inf) = NaN and arg < 0 (lg2 = NaN) gives NaN with no compare and no select.
+// Measured against the oracle's stage 5: max 1.7e-6 mag (fp64 finish: 1.6e-6).  A flux below FLT_MIN (1.2e-38: fainter
+// than zp + 94.8 mag) is flushed to zero by the .ftz form and gives NaN (DESIGN.md R-Q20).
 __device__ __forceinline__ float mag_of(float arg, double zp) {
-    // branch-free: the 16 magnitudes of a thread are independent chains the scheduler can interleave
-    // zp and -2.5 log10(2) as float pairs: two fp32 FMAs instead of float->double, fp64 FMA, double->float (the conversion
-    // unit is a scarce pipe here).  Measured against the oracle's stage 5: max 1.7e-6 mag (fp64 finish: 1.6e-6).
     const float zph = (float)zp, zpl = (float)(zp - (double)zph);
     float l2;
-    asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(l2) : "f"(fmaxf(arg, 1.17549435e-38f)));   // a denormal flux is not flushed to -inf
-    const float mg = fmaf(l2, -0.752574980258941650390625f, zph) + fmaf(l2, -8.901011e-9f, zpl);
-    return arg > 0.f ? mg : __int_as_float(0x7fc00000);
+    asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(l2) : "f"(arg));
+    return fmaf(l2, -0.75257503986358642578125f, zph) + fmaf(l2, 5.0703633e-8f, zpl);
 }
 __device__ __forceinline__ float sqrt_approx(float x) {
     float r;
@@ -295,9 +296,9 @@ __global__ void __launch_bounds__(C2_THREADS, (NOISE ? 4 : C2_MINB_CLEAN)) k_con
     static_assert((C2_TW / 4 - 1 + NV) * 4 <= SW, "row-pass window leaves the halo row");
     static_assert(C2_TH - 4 + K + 2 < SH, "column-pass window leaves the halo tile");
     extern __shared__ __align__(16) float sm[];
-    float *tile = sm;                             // [SH][SW]
+    float *tile = sm;                             // [SH + 1][SW]: row SH is a spare row nobody writes (row pass, idle lanes)
     float *hrow = sm;                             // row results overwrite the first 64 columns of their own tile row (stride SW)
-    uint32_t *ssky = reinterpret_cast<uint32_t *>(sm + SH * SW);        // [SKY_CAP], noisy instances only
+    uint32_t *ssky = reinterpret_cast<uint32_t *>(sm + (SH + 1) * SW);        // [SKY_CAP], noisy instances only
     const int N = a.N, m = blockIdx.z, mb = m * a.B + a.band, tid = threadIdx.x;
     const float *F = a.F + (size_t)mb * a.P;
     const int x0 = blockIdx.x * C2_TW, y0 = blockIdx.y * C2_TH;
@@ -367,7 +368,8 @@ __global__ void __launch_bounds__(C2_THREADS, (NOISE ? 4 : C2_MINB_CLEAN)) k_con
         float v[NV * 4];
 #pragma unroll
         for (int q = 0; q < NV; ++q) {
-            const float4 f4 = live ? reinterpret_cast<const float4 *>(tile + i * SW)[sgm + q] : make_float4(0.f, 0.f, 0.f, 0.f);
+            // idle lanes read the spare row (values unused): an unconditional load, no zero-filling of the window
+            const float4 f4 = reinterpret_cast<const float4 *>(tile + (live ? i : SH) * SW)[sgm + q];
             v[4 * q] = f4.x; v[4 * q + 1] = f4.y; v[4 * q + 2] = f4.z; v[4 * q + 3] = f4.w;
         }
         // h[c] = sum_i fr[b - i] v[i], i = OFF + c ... OFF + c + K - 1, b = OFF + c + K - 1: aligned input pairs
@@ -471,7 +473,7 @@ __global__ void __launch_bounds__(C2_THREADS, (NOISE ? 4 : C2_MINB_CLEAN)) k_con
 template <int K>
 static size_t conv2_smem(bool noise) {
     constexpr int R = (K - 1) / 2, RA = (R + 3) & ~3;
-    return ((size_t)(C2_TH + K - 1) * (C2_TW + 2 * RA) + (noise ? 1024 : 0)) * sizeof(float);
+    return ((size_t)(C2_TH + K - 1 + 1) * (C2_TW + 2 * RA) + (noise ? 1024 : 0)) * sizeof(float);   // + the spare row
 }
 
 template <int K>

@@ -46,3 +46,54 @@ def test_batched_separable_convolution_and_noise(cfg, K, sig, n_im, n_models):
         assert np.max(np.abs(mag[ok] - want[ok])) <= MAG_ATOL
     g.debug_taps(None, None)
     g.close()
+
+
+@pytest.mark.parametrize("read_sigma", [0.0, 3.0])
+def test_batched_magnitude_of_non_positive_flux_is_nan(read_sigma):
+    """Stage 5 on k_conv2 for fluxes <= 0 (R-Q11: the magnitude of a non-positive flux is NaN): a model without stars
+    (every flux exactly 0: lg2 = -inf, the kernel's NaN comes out of (+inf) + (-inf), csrc/conv_noise.cu mag_of) and, with
+    read noise and no sky, a sparse model whose noisy fluxes are negative in about half of the empty pixels."""
+    import torch
+    import paper_1904_00011_b200 as G
+    base = W.config(1)
+    wl = dict(W.with_psf(W.scaled(base, 64), 7, [1.0] * int(base["n_bands"])))
+    wl["sky"] = np.zeros_like(wl["sky"])
+    wl["read_sigma"] = np.full_like(wl["read_sigma"], read_sigma)
+    wl["shot_noise"], wl["poisson_sky"] = 0, 0
+    n_models = 300
+    p0 = wl["params"][0]
+    prm = [dict(p0, sfh=np.asarray(p0["sfh"]) * (0.0 if i % 2 == 0 else 1e-4)) for i in range(n_models)]
+    g = G.Pcmd(wl, separable=True)
+    P = g.N * g.N
+    fc = torch.empty((n_models, g.B, g.N, g.N), dtype=torch.float32, device="cuda")
+    g.debug_taps(None, fc)
+    seed, m0 = 31, 2
+    out = g.simulate(prm, seed=seed, model_index0=m0)
+    torch.cuda.synchronize()
+    assert g.status() == 0
+    orc = O.Oracle(wl)
+    n_nan = 0
+    for i in (0, 1, n_models - 2, n_models - 1):
+        got = fc[i].cpu().numpy().reshape(g.B, P)
+        if i % 2 == 0:
+            assert not got.any()                                            # no stars: flux exactly zero everywhere
+        want = orc.stage5(got.astype(np.float64), seed, model=m0 + i)
+        mag = out["mag"][i].cpu().numpy().reshape(g.B, P)
+        ok = ~np.isnan(want)
+        assert np.array_equal(np.isnan(mag), ~ok)
+        assert not np.isinf(mag).any()
+        if ok.any():
+            # a flux that is the noise draw alone (|flux| << sigma) is ill-conditioned in magnitudes (d mag = 1.09 d flux /
+            # flux, d flux = sigma x the fp32 error of the normal draw): compare it as a flux, on the scale of sigma
+            zp = np.asarray(wl["zp"], dtype=np.float64)[:, None]
+            f_got, f_want = 10.0 ** (-0.4 * (mag - zp)), 10.0 ** (-0.4 * (want - zp))
+            assert np.max(np.abs(f_got[ok] - f_want[ok]) - FLUX_RTOL * np.abs(f_want[ok])) <= 1e-5 * max(read_sigma, 1e-30)
+            well = ok & (f_want > max(read_sigma, 1e-30))
+            if well.any():
+                assert np.max(np.abs(mag[well] - want[well])) <= MAG_ATOL
+        n_nan += int((~ok).sum())
+        if read_sigma == 0.0 and i % 2 == 0:
+            assert not ok.any()
+    assert n_nan > P                                                        # the case is exercised
+    g.debug_taps(None, None)
+    g.close()
