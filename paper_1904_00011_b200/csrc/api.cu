@@ -21,6 +21,12 @@ static int upload(pcmd_ctx *c, T **dst, const T *src, size_t n) {
     return PCMD_OK;
 }
 
+int pcmd_pdl_enabled() {
+    static int on = -1;
+    if (on < 0) { const char *e = getenv("PCMD_NO_PDL"); on = (e && e[0] == '1') ? 0 : 1; }
+    return on;
+}
+
 extern "C" const char *pcmd_strerror(int code) {
     switch (code) {
         case PCMD_OK: return "ok";

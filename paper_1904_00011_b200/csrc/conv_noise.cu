@@ -35,6 +35,7 @@ __device__ __forceinline__ void noise_mag_epilogue(const CvArgs &a, const float 
                                                    int lx, int m, int b, int mb);
 
 __global__ void __launch_bounds__(CV_TX * CV_ROWS) k_conv_noise(const CvArgs a) {
+    pdl_enter();
     extern __shared__ float sm[];
     const int K = a.K, r = (K - 1) / 2, N = a.N;
     const int TW = CV_TX + K - 1, TH = CV_TY + K - 1;
@@ -94,6 +95,7 @@ __global__ void __launch_bounds__(CV_TX * CV_ROWS) k_conv_noise(const CvArgs a) 
 // memory, then the column pass: 2K FMAs per output instead of K^2.  Same tile, halo and epilogue.
 template <int KT>
 __global__ void __launch_bounds__(CV_TX * CV_ROWS) k_conv_noise_sep(const CvArgs a) {
+    pdl_enter();
     extern __shared__ float sm[];
     const int K = KT ? KT : a.K, r = (K - 1) / 2, N = a.N;
     const int TW = CV_TX + K - 1, TH = CV_TY + K - 1;
@@ -288,6 +290,7 @@ __device__ __forceinline__ float noise_mag_one(const Cv2Args &a, float Gi, uint3
 // NOISE = false: no shot / read noise and no Poisson sky (stage 5 is the magnitude only): a leaner instance
 template <int K, bool VEC, bool NOISE>
 __global__ void __launch_bounds__(C2_THREADS, (NOISE ? 4 : C2_MINB_CLEAN)) k_conv2(const Cv2Args a) {
+    pdl_enter();
     constexpr int R = (K - 1) / 2, RA = (R + 3) & ~3, OFF = RA - R;
     constexpr int SW = C2_TW + 2 * RA;            // halo-tile row stride (floats), a multiple of 4
     constexpr int SH = C2_TH + K - 1;             // halo-tile rows
@@ -482,10 +485,10 @@ static cudaError_t conv2_launch(const Cv2Args &a, int n_models, cudaStream_t s) 
     const bool vec = (a.N & 3) == 0 && ((reinterpret_cast<uintptr_t>(a.F) | reinterpret_cast<uintptr_t>(a.mag) |
                                          reinterpret_cast<uintptr_t>(a.tap_conv)) & 15) == 0;
     const bool noise = a.shot_noise || a.read_sigma > 0.0 || (a.poisson_sky && a.sky > 0.0);
-    if (vec && noise) k_conv2<K, true, true><<<grid, C2_THREADS, conv2_smem<K>(true), s>>>(a);
-    else if (vec) k_conv2<K, true, false><<<grid, C2_THREADS, conv2_smem<K>(false), s>>>(a);
-    else if (noise) k_conv2<K, false, true><<<grid, C2_THREADS, conv2_smem<K>(true), s>>>(a);
-    else k_conv2<K, false, false><<<grid, C2_THREADS, conv2_smem<K>(false), s>>>(a);
+    if (vec && noise) pcmd_launch_pdl((k_conv2<K, true, true>), grid, dim3(C2_THREADS), conv2_smem<K>(true), s, a);
+    else if (vec) pcmd_launch_pdl((k_conv2<K, true, false>), grid, dim3(C2_THREADS), conv2_smem<K>(false), s, a);
+    else if (noise) pcmd_launch_pdl((k_conv2<K, false, true>), grid, dim3(C2_THREADS), conv2_smem<K>(true), s, a);
+    else pcmd_launch_pdl((k_conv2<K, false, false>), grid, dim3(C2_THREADS), conv2_smem<K>(false), s, a);
     return cudaGetLastError();
 }
 
@@ -542,16 +545,16 @@ int pcmd_launch_conv_noise(pcmd_ctx *c, int n_models, uint64_t seed, uint32_t mo
     if (c->psf_sep) {
         size_t smem = ((size_t)(CV_TX + K - 1) * (CV_TY + K - 1) + (size_t)(CV_TY + K - 1) * CV_TX + 2 * (size_t)K) * sizeof(float);
         const dim3 blk(CV_TX, CV_ROWS);
-        if (K == 5) k_conv_noise_sep<5><<<grid, blk, smem, s>>>(a);
-        else if (K == 7) k_conv_noise_sep<7><<<grid, blk, smem, s>>>(a);
-        else if (K == 15) k_conv_noise_sep<15><<<grid, blk, smem, s>>>(a);
-        else if (K == 21) k_conv_noise_sep<21><<<grid, blk, smem, s>>>(a);
+        if (K == 5) pcmd_launch_pdl((k_conv_noise_sep<5>), grid, blk, smem, s, a);
+        else if (K == 7) pcmd_launch_pdl((k_conv_noise_sep<7>), grid, blk, smem, s, a);
+        else if (K == 15) pcmd_launch_pdl((k_conv_noise_sep<15>), grid, blk, smem, s, a);
+        else if (K == 21) pcmd_launch_pdl((k_conv_noise_sep<21>), grid, blk, smem, s, a);
         else {
             if (smem > 48 * 1024 && smem > c->smem_conv_sep) {
                 PCMD_CUDA(c, cudaFuncSetAttribute(k_conv_noise_sep<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
                 c->smem_conv_sep = smem;
             }
-            k_conv_noise_sep<0><<<grid, blk, smem, s>>>(a);
+            pcmd_launch_pdl((k_conv_noise_sep<0>), grid, blk, smem, s, a);
         }
     } else {
         size_t smem = ((size_t)(CV_TX + K - 1) * (CV_TY + K - 1) + (size_t)K * K) * sizeof(float);
@@ -559,7 +562,7 @@ int pcmd_launch_conv_noise(pcmd_ctx *c, int n_models, uint64_t seed, uint32_t mo
             PCMD_CUDA(c, cudaFuncSetAttribute(k_conv_noise, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
             c->smem_conv = smem;
         }
-        k_conv_noise<<<grid, dim3(CV_TX, CV_ROWS), smem, s>>>(a);
+        pcmd_launch_pdl(k_conv_noise, grid, dim3(CV_TX, CV_ROWS), smem, s, a);
     }
     PCMD_LAUNCHED(c);
     return PCMD_OK;

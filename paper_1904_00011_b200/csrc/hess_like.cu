@@ -16,6 +16,7 @@ __global__ void __launch_bounds__(HS_THREADS) k_hess(const float *__restrict__ m
                                                      int64_t bins_total, uint32_t *__restrict__ hess,
                                                      pcmd_hess_stats *__restrict__ part,
                                                      pcmd_hess_stats *__restrict__ stats_out) {
+    pdl_enter();
     extern __shared__ uint32_t sh[];
     const int h = blockIdx.y, m = blockIdx.z;
     const DevHess S = specs[h];
@@ -109,6 +110,7 @@ __global__ void __launch_bounds__(HS_THREADS) k_hess(const float *__restrict__ m
 
 __global__ void k_hess_stats(const pcmd_hess_stats *__restrict__ part, int nblk,
                              pcmd_hess_stats *__restrict__ out) {
+    pdl_enter();
     // one warp per (model, hess): lane l adds partials l, l+32, ... in order, then a shuffle tree
     // (a fixed order: deterministic sums)
     const pcmd_hess_stats *p = part + (size_t)blockIdx.x * nblk;
@@ -162,15 +164,15 @@ int pcmd_launch_hess(pcmd_ctx *c, const float *d_mag, int n_models, uint32_t *d_
             PCMD_CUDA(c, cudaFuncSetAttribute(k_hess<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
             c->smem_hess = smem;
         }
-        k_hess<true><<<grid, HS_THREADS, smem, s>>>(d_mag, c->B, c->P, c->d_hess_spec, c->n_hess, ppb,
+        pcmd_launch_pdl((k_hess<true>), grid, dim3(HS_THREADS), smem, s, d_mag, c->B, c->P, c->d_hess_spec, c->n_hess, ppb,
                                                     c->hess_bins, d_hess, c->d_hpart, d_stats);
     } else {
-        k_hess<false><<<grid, HS_THREADS, 0, s>>>(d_mag, c->B, c->P, c->d_hess_spec, c->n_hess, ppb,
+        pcmd_launch_pdl((k_hess<false>), grid, dim3(HS_THREADS), 0, s, d_mag, c->B, c->P, c->d_hess_spec, c->n_hess, ppb,
                                                   c->hess_bins, d_hess, c->d_hpart, d_stats);
     }
     PCMD_LAUNCHED(c);
     if (d_stats && nblk > 1) {
-        k_hess_stats<<<n_models * c->n_hess, 32, 0, s>>>(c->d_hpart, nblk, d_stats);
+        pcmd_launch_pdl(k_hess_stats, dim3(n_models * c->n_hess), dim3(32), 0, s, c->d_hpart, nblk, d_stats);
         PCMD_LAUNCHED(c);
     }
     return PCMD_OK;
@@ -213,6 +215,7 @@ __global__ void __launch_bounds__(LL_THREADS) k_loglike(const uint32_t *__restri
                                                         int64_t bins_total, int mode, double m_floor,
                                                         const double *__restrict__ lfact,
                                                         double *__restrict__ out) {
+    pdl_enter();
     __shared__ double scratch[LL_THREADS / 32];
     const int m = blockIdx.x;
     double total = 0.0;
@@ -261,7 +264,7 @@ __global__ void __launch_bounds__(LL_THREADS) k_loglike(const uint32_t *__restri
 int pcmd_launch_loglike(pcmd_ctx *c, const uint32_t *d_hm, const pcmd_hess_stats *d_sm, int n_models,
                         const uint32_t *d_hd, const pcmd_hess_stats *d_sd, int mode, double *d_out,
                         cudaStream_t s) {
-    k_loglike<<<n_models, LL_THREADS, 0, s>>>(d_hm, d_sm, d_hd, d_sd, c->d_hess_spec, c->n_hess,
+    pcmd_launch_pdl(k_loglike, dim3(n_models), dim3(LL_THREADS), 0, s, d_hm, d_sm, d_hd, d_sd, c->d_hess_spec, c->n_hess,
                                               c->hess_bins, mode, c->like_floor, c->d_lfact, d_out);
     PCMD_LAUNCHED(c);
     return PCMD_OK;
@@ -338,15 +341,15 @@ extern "C" int pcmd_hess_noalloc(pcmd_ctx *c, const float *d_mag, int32_t n_mode
             PCMD_CUDA(c, cudaFuncSetAttribute(k_hess<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
             c->smem_hess = smem;
         }
-        k_hess<true><<<grid, HS_THREADS, smem, s>>>(d_mag, c->B, c->P, c->d_hess_spec, c->n_hess, ppb,
+        pcmd_launch_pdl((k_hess<true>), grid, dim3(HS_THREADS), smem, s, d_mag, c->B, c->P, c->d_hess_spec, c->n_hess, ppb,
                                                     c->hess_bins, d_hess, parts, d_stats);
     } else {
-        k_hess<false><<<grid, HS_THREADS, 0, s>>>(d_mag, c->B, c->P, c->d_hess_spec, c->n_hess, ppb,
+        pcmd_launch_pdl((k_hess<false>), grid, dim3(HS_THREADS), 0, s, d_mag, c->B, c->P, c->d_hess_spec, c->n_hess, ppb,
                                                   c->hess_bins, d_hess, parts, d_stats);
     }
     PCMD_LAUNCHED(c);
     if (d_stats && nblk > 1) {
-        k_hess_stats<<<n_models * c->n_hess, 32, 0, s>>>(parts, nblk, d_stats);
+        pcmd_launch_pdl(k_hess_stats, dim3(n_models * c->n_hess), dim3(32), 0, s, parts, nblk, d_stats);
         PCMD_LAUNCHED(c);
     }
     PCMD_PROF(c, 5, s);

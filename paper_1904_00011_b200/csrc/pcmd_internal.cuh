@@ -181,6 +181,33 @@ struct pcmd_ctx {
         }                                                                 \
     } while (0)
 
+// Programmatic dependent launch (PDL) -------------------------------------------------------
+// The kernels of one evaluation form a chain on the caller's stream, and on small jobs (c1: 64 x 64 pixels) the
+// launch latency between them is a large part of the step.  Every kernel of the chain starts with pdl_enter():
+// griddepcontrol.wait (returns once the previous kernel of the stream has completed and its writes are visible;
+// a no-op for a kernel launched without the attribute) followed by griddepcontrol.launch_dependents (lets the
+// NEXT kernel, if it was launched with the attribute, be set up and made resident while this one runs; it then
+// sits in its own wait).  Completion is transitive along the chain because every kernel waits before it does
+// anything else.  pcmd_launch_pdl launches with cudaLaunchAttributeProgrammaticStreamSerialization; only
+// kernels that begin with pdl_enter() may be launched through it.  PCMD_NO_PDL=1 in the environment switches
+// the attribute off (plain stream order).
+__device__ __forceinline__ void pdl_enter() {
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+}
+int pcmd_pdl_enabled();     // api.cu
+template <typename... KA, typename... A>
+static inline cudaError_t pcmd_launch_pdl(void (*kern)(KA...), dim3 grid, dim3 block, size_t smem, cudaStream_t s,
+                                          A &&...args) {
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = s;
+    cfg.attrs = at; cfg.numAttrs = pcmd_pdl_enabled() ? 1 : 0;
+    return cudaLaunchKernelEx(&cfg, kern, static_cast<A &&>(args)...);
+}
+
 // error helpers ---------------------------------------------------------------------------
 #define PCMD_CUDA(ctx, call)                                              \
     do {                                                                  \

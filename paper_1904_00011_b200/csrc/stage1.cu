@@ -245,6 +245,7 @@ __constant__ uint32_t c_s2_group_cost[S2_NCLASS] = {S2_COST_G, S2_COST_D9, S2_CO
 __global__ void __launch_bounds__(1024) k_group_sort(const uint8_t *__restrict__ cls_all, int Jpad,
                                                      int64_t arena_cap, uint32_t *__restrict__ pos_all,
                                                      ModelPlan *__restrict__ plan_all) {
+    pdl_enter();
     __shared__ uint32_t wcnt[32][S2_NCLASS];
     __shared__ uint32_t count[S2_NCLASS + 1], carry[S2_NCLASS], cls_start[S2_NCLASS + 1];
     const int m = blockIdx.x, n_groups = Jpad >> 2;
@@ -337,6 +338,7 @@ __global__ void __launch_bounds__(128) k_points(const DevModel *__restrict__ mdl
                          double *__restrict__ qbuf, int64_t cap, uint32_t *__restrict__ tab_all,
                          uint32_t *__restrict__ alloc, PointRec *__restrict__ rec_out,
                          uint8_t *__restrict__ gcls_out, int32_t *status) {
+    pdl_enter();
     extern __shared__ double w[];  // [Z]
     const int m = blockIdx.y;
     const DevModel M = mdl[m];
@@ -441,6 +443,7 @@ __global__ void __launch_bounds__(256) k_group_emit(const PointRec *__restrict__
                                                     const uint32_t *__restrict__ pos_all,
                                                     const ModelPlan *__restrict__ plan_all, GroupRec *__restrict__ grp_all,
                                                     uint32_t *__restrict__ arena_all, int64_t arena_cap) {
+    pdl_enter();
     const int m = blockIdx.y, n_groups = Jpad >> 2, lane = threadIdx.x & 31;
     const int g = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
     if (g >= n_groups) return;
@@ -515,14 +518,14 @@ int pcmd_launch_stage1(pcmd_ctx *c, int n_models, cudaStream_t s) {
         return pcmd_launch_agg_tables(c, n_models, s);
     }
     PCMD_CUDA(c, cudaMemsetAsync(c->d_alloc, 0, (size_t)n_models * 2 * sizeof(uint32_t), s));
-    k_points<<<dim3((c->Jpad + 127) / 128, n_models), 128, c->Z * sizeof(double), s>>>(
+    pcmd_launch_pdl(k_points, dim3((c->Jpad + 127) / 128, n_models), dim3(128), c->Z * sizeof(double), s, 
         c->d_model, c->d_sfh, c->d_feh_grid, c->d_age_idx, c->d_feh_idx, c->d_imf_w, c->d_absmag, c->A, c->Z, c->J,
         c->Jpad, c->B, c->mdf_cut, c->zp[0], c->zp[1], c->zp[2], c->zp[3], c->d_mdfw, c->d_lambda, c->d_q,
         c->cap_raw, c->d_tab, c->d_alloc, c->d_rec, c->d_gcls, c->d_status);
     PCMD_LAUNCHED(c);
-    k_group_sort<<<n_models, 1024, 0, s>>>(c->d_gcls, c->Jpad, c->arena_cap, c->d_gpos, c->d_plan);
+    pcmd_launch_pdl(k_group_sort, dim3(n_models), dim3(1024), 0, s, c->d_gcls, c->Jpad, c->arena_cap, c->d_gpos, c->d_plan);
     PCMD_LAUNCHED(c);
-    k_group_emit<<<dim3((n_groups + 7) / 8, n_models), 256, 0, s>>>(c->d_rec, c->d_tab, c->cap_raw, c->Jpad, c->d_gcls,
+    pcmd_launch_pdl(k_group_emit, dim3((n_groups + 7) / 8, n_models), dim3(256), 0, s, c->d_rec, c->d_tab, c->cap_raw, c->Jpad, c->d_gcls,
                                                                     c->d_gpos, c->d_plan, c->d_grp, c->d_arena,
                                                                     c->arena_cap);
     PCMD_LAUNCHED(c);

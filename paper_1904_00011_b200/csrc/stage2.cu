@@ -439,6 +439,7 @@ __device__ __forceinline__ void s2_issue(const S2Args &a, S2Shared &sh, GroupRec
 // ---- the persistent kernel ----------------------------------------------------------------------
 template <int NB, bool COUNTS>
 __global__ void __launch_bounds__(S2_THREADS, S2_MINB) k_stage2(const S2Args a) {
+    pdl_enter();
     extern __shared__ __align__(128) unsigned char s2_smem[];
     GroupRec *sbuf = reinterpret_cast<GroupRec *>(s2_smem);                                     // [S2_NST][S2_CHUNK]
     uint32_t *stab = reinterpret_cast<uint32_t *>(s2_smem + (size_t)S2_NST * S2_CHUNK * sizeof(GroupRec));   // [S2_NST][S2_TABW]
@@ -576,6 +577,7 @@ struct RdArgs {
 };
 
 __global__ void __launch_bounds__(256) k_reduce_dust(const RdArgs a) {
+    pdl_enter();
     const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (idx >= a.P * a.n_models) return;
     const int m = (int)(idx / a.P);
@@ -624,8 +626,8 @@ int pcmd_stage2_segments(const pcmd_ctx *c, int n_models) {
 
 template <int NB>
 static cudaError_t launch_s2(const S2Args &a, bool counts, int grid, cudaStream_t s) {
-    if (counts) k_stage2<NB, true><<<grid, S2_THREADS, s2_smem_bytes(), s>>>(a);
-    else k_stage2<NB, false><<<grid, S2_THREADS, s2_smem_bytes(), s>>>(a);
+    if (counts) pcmd_launch_pdl((k_stage2<NB, true>), grid, dim3(S2_THREADS), s2_smem_bytes(), s, a);
+    else pcmd_launch_pdl((k_stage2<NB, false>), grid, dim3(S2_THREADS), s2_smem_bytes(), s, a);
     return cudaGetLastError();
 }
 
@@ -666,7 +668,7 @@ int pcmd_launch_stage2(pcmd_ctx *c, int n_models, uint64_t seed, uint32_t model0
     r.key0 = a.key0; r.key1 = a.key1; r.model0 = model0; r.dust_frac = c->dust_frac;
     for (int b = 0; b < 4; ++b) r.coef[b] = c->dust_coef[b];
     const int64_t n = c->P * n_models;
-    k_reduce_dust<<<(unsigned)((n + 255) / 256), 256, 0, s>>>(r);
+    pcmd_launch_pdl(k_reduce_dust, dim3((unsigned)((n + 255) / 256)), dim3(256), 0, s, r);
     PCMD_LAUNCHED(c);
     return PCMD_OK;
 }
