@@ -6,12 +6,15 @@
 #ifndef HS_THREADS
 #define HS_THREADS 512
 #endif
+#ifndef HS_MINB
+#define HS_MINB 1
+#endif
 #define HS_PIX_PER_BLOCK 4096
 
 // Binning arithmetic, fp32, no contraction:
 // x = fl(mp - mm); t = fl(fl(x - x_lo) * inv_dx); ix = floor(t); half-open.
 template <bool SMEM>
-__global__ void __launch_bounds__(HS_THREADS) k_hess(const float *__restrict__ mag, int B, int64_t P,
+__global__ void __launch_bounds__(HS_THREADS, HS_MINB) k_hess(const float *__restrict__ mag, int B, int64_t P,
                                                      const DevHess *__restrict__ specs, int n_hess, int64_t ppb,
                                                      int64_t bins_total, uint32_t *__restrict__ hess,
                                                      pcmd_hess_stats *__restrict__ part,
@@ -23,7 +26,7 @@ __global__ void __launch_bounds__(HS_THREADS) k_hess(const float *__restrict__ m
     const int nbins = S.nx * S.ny;
     uint32_t *gh = hess + (size_t)m * bins_total + S.bin_off;
     if (SMEM) {
-        for (int t = threadIdx.x; t < nbins; t += HS_THREADS) sh[t] = 0;
+        for (int t = threadIdx.x; t < nbins + 2; t += HS_THREADS) sh[t] = 0;      // + the spare counters sh[nbins], sh[nbins + 1]
         __syncthreads();
     }
     const float *mp = mag + ((size_t)m * B + S.band_plus) * P;
@@ -34,28 +37,48 @@ __global__ void __launch_bounds__(HS_THREADS) k_hess(const float *__restrict__ m
     const int64_t p0 = (int64_t)blockIdx.x * ppb;
     const int64_t p1 = min(P, p0 + ppb);
     auto one = [&](float a, float b, float y) {
-        if (isnan(a) || isnan(b) || isnan(y)) { n_bad++; return; }
         const float x = __fsub_rn(a, b);
         // floor and conversion in one instruction (saturating, so a far-out value stays out); 0 <= ix < nx as one
         // unsigned compare: the same decision as floorf + float range test
         const int ix = __float2int_rd(__fmul_rn(__fsub_rn(x, S.x_lo), S.inv_dx));
         const int iy = __float2int_rd(__fmul_rn(__fsub_rn(y, S.y_lo), S.inv_dy));
-        if ((unsigned)ix >= (unsigned)S.nx || (unsigned)iy >= (unsigned)S.ny) { n_out++; return; }
-        const int bin = iy * S.nx + ix;
-        PCMD_CHK(bin >= 0 && bin < nbins);
-        if (SMEM) atomicAdd(&sh[bin], 1u); else atomicAdd(&gh[bin], 1u);
-        n_in++; sx += (double)x; sy += (double)y;
+        if (SMEM) {
+            // branch-free (a warp's pixels rarely agree, and a branch per pixel costs its compare, its reconvergence
+            // pair and the tail of the block around it): a pixel outside the window goes to the spare counter
+            // sh[nbins], a NaN pixel to sh[nbins + 1] (the conversion gives 0 for NaN, so NaN is tested apart: both
+            // scaled coordinates in one two-operand test -- NaN propagates from a, b and y into them), and both add
+            // 0.0 to the sums; n_out, n_bad and n_in come out of the two counters and the block's pixel count (below)
+            const float tx = __fmul_rn(__fsub_rn(x, S.x_lo), S.inv_dx), ty = __fmul_rn(__fsub_rn(y, S.y_lo), S.inv_dy);
+            int bad;
+            asm("{\n.reg .pred p;\nsetp.nan.f32 p, %1, %2;\nselp.s32 %0, 1, 0, p;\n}" : "=r"(bad) : "f"(tx), "f"(ty));
+            const bool in = !bad && (unsigned)ix < (unsigned)S.nx && (unsigned)iy < (unsigned)S.ny;
+            const int bin = in ? iy * S.nx + ix : nbins + bad;
+            PCMD_CHK(bin >= 0 && bin <= nbins + 1);
+            atomicAdd(&sh[bin], 1u);
+            // the select is taken on the fp32 bit pattern, before the conversion (one select, not two on the halves of a double)
+            sx += (double)__uint_as_float(in ? __float_as_uint(x) : 0u);
+            sy += (double)__uint_as_float(in ? __float_as_uint(y) : 0u);
+        } else {
+            if (isnan(a) || isnan(b) || isnan(y)) { n_bad++; return; }
+            if ((unsigned)ix >= (unsigned)S.nx || (unsigned)iy >= (unsigned)S.ny) { n_out++; return; }
+            const int bin = iy * S.nx + ix;
+            PCMD_CHK(bin >= 0 && bin < nbins);
+            atomicAdd(&gh[bin], 1u);
+            n_in++; sx += (double)x; sy += (double)y;
+        }
     };
     if (((P | p0) & 3) == 0 && (reinterpret_cast<uintptr_t>(mag) & 15) == 0) {      // 16-byte loads: every band of every image starts 16-byte aligned
         const float4 *vp = reinterpret_cast<const float4 *>(mp), *vm = reinterpret_cast<const float4 *>(mm),
                      *vy = reinterpret_cast<const float4 *>(my);
         const int64_t q1 = (p1 + 3) >> 2;
+        PCMD_CHK((p1 & 3) == 0);
         const bool y_is_minus = (my == mm), y_is_plus = (my == mp);    // the usual case: y is one of the colour's bands
         auto four = [&](int64_t q, const float4 &A, const float4 &Bv, const float4 &Y) {
+            // P, p0 and ppb are multiples of 4 here: every quad of the block's range is a full one
             one(A.x, Bv.x, Y.x);
-            if (4 * q + 1 < p1) one(A.y, Bv.y, Y.y);
-            if (4 * q + 2 < p1) one(A.z, Bv.z, Y.z);
-            if (4 * q + 3 < p1) one(A.w, Bv.w, Y.w);
+            one(A.y, Bv.y, Y.y);
+            one(A.z, Bv.z, Y.z);
+            one(A.w, Bv.w, Y.w);
         };
         int64_t q = (p0 >> 2) + threadIdx.x;
         for (; q + HS_THREADS < q1; q += 2 * HS_THREADS) {             // two 16-byte loads per band in flight
@@ -93,6 +116,7 @@ __global__ void __launch_bounds__(HS_THREADS) k_hess(const float *__restrict__ m
             st.n_in += r_n[0][w]; st.n_out += r_n[1][w]; st.n_bad += r_n[2][w];
             st.sum_x += r_sx[w]; st.sum_y += r_sy[w];
         }
+        if (SMEM) { st.n_out = sh[nbins]; st.n_bad = sh[nbins + 1]; st.n_in = (uint32_t)(p1 - p0) - st.n_out - st.n_bad; }
         if (gridDim.x == 1 && stats_out) stats_out[(size_t)m * n_hess + h] = st;   // the only block: final stats
         else part[((size_t)m * n_hess + h) * gridDim.x + blockIdx.x] = st;
     }
@@ -155,7 +179,7 @@ int pcmd_launch_hess(pcmd_ctx *c, const float *d_mag, int n_models, uint32_t *d_
     }
     int maxbins = 0;
     for (int h = 0; h < c->n_hess; ++h) maxbins = max(maxbins, c->hess[h].nx * c->hess[h].ny);
-    size_t smem = (size_t)maxbins * sizeof(uint32_t);
+    size_t smem = ((size_t)maxbins + 2) * sizeof(uint32_t);      // + the two spare counters
     if (!(nblk == 1 && smem <= 200 * 1024))    // a single block per diagram stores its histogram itself
         PCMD_CUDA(c, cudaMemsetAsync(d_hess, 0, (size_t)n_models * c->hess_bins * sizeof(uint32_t), s));
     dim3 grid(nblk, c->n_hess, n_models);
@@ -331,7 +355,7 @@ extern "C" int pcmd_hess_noalloc(pcmd_ctx *c, const float *d_mag, int32_t n_mode
     PCMD_CUDA(c, hess_noalloc_addr(&parts));
     int maxbins = 0;
     for (int h = 0; h < c->n_hess; ++h) maxbins = max(maxbins, c->hess[h].nx * c->hess[h].ny);
-    const size_t smem = (size_t)maxbins * sizeof(uint32_t);
+    const size_t smem = ((size_t)maxbins + 2) * sizeof(uint32_t);      // + the two spare counters
     PCMD_PROF(c, 4, s);
     if (!(nblk == 1 && smem <= 200 * 1024))
         PCMD_CUDA(c, cudaMemsetAsync(d_hess, 0, (size_t)n_models * c->hess_bins * sizeof(uint32_t), s));
