@@ -7,14 +7,15 @@
 #define HS_THREADS 512
 #endif
 #ifndef HS_MINB
-#define HS_MINB 1
+#define HS_MINB 2        // blocks per SM of the 512-thread instance (64-register cap; without it the compiler takes 96 registers: one block per SM)
 #endif
 #define HS_PIX_PER_BLOCK 4096
 
 // Binning arithmetic, fp32, no contraction:
 // x = fl(mp - mm); t = fl(fl(x - x_lo) * inv_dx); ix = floor(t); half-open.
-template <bool SMEM>
-__global__ void __launch_bounds__(HS_THREADS, HS_MINB) k_hess(const float *__restrict__ mag, int B, int64_t P,
+// NT threads per block: HS_THREADS, or 1024 when the histogram leaves room for one block per SM only
+template <bool SMEM, int NT>
+__global__ void __launch_bounds__(NT, (NT == HS_THREADS ? HS_MINB : 1)) k_hess(const float *__restrict__ mag, int B, int64_t P,
                                                      const DevHess *__restrict__ specs, int n_hess, int64_t ppb,
                                                      int64_t bins_total, uint32_t *__restrict__ hess,
                                                      pcmd_hess_stats *__restrict__ part,
@@ -26,7 +27,7 @@ __global__ void __launch_bounds__(HS_THREADS, HS_MINB) k_hess(const float *__res
     const int nbins = S.nx * S.ny;
     uint32_t *gh = hess + (size_t)m * bins_total + S.bin_off;
     if (SMEM) {
-        for (int t = threadIdx.x; t < nbins + 2; t += HS_THREADS) sh[t] = 0;      // + the spare counters sh[nbins], sh[nbins + 1]
+        for (int t = threadIdx.x; t < nbins + 2; t += NT) sh[t] = 0;      // + the spare counters sh[nbins], sh[nbins + 1]
         __syncthreads();
     }
     const float *mp = mag + ((size_t)m * B + S.band_plus) * P;
@@ -81,24 +82,24 @@ __global__ void __launch_bounds__(HS_THREADS, HS_MINB) k_hess(const float *__res
             one(A.w, Bv.w, Y.w);
         };
         int64_t q = (p0 >> 2) + threadIdx.x;
-        for (; q + HS_THREADS < q1; q += 2 * HS_THREADS) {             // two 16-byte loads per band in flight
-            const float4 A0 = vp[q], B0 = vm[q], A1 = vp[q + HS_THREADS], B1 = vm[q + HS_THREADS];
+        for (; q + NT < q1; q += 2 * NT) {             // two 16-byte loads per band in flight
+            const float4 A0 = vp[q], B0 = vm[q], A1 = vp[q + NT], B1 = vm[q + NT];
             const float4 Y0 = y_is_minus ? B0 : (y_is_plus ? A0 : vy[q]);
-            const float4 Y1 = y_is_minus ? B1 : (y_is_plus ? A1 : vy[q + HS_THREADS]);
+            const float4 Y1 = y_is_minus ? B1 : (y_is_plus ? A1 : vy[q + NT]);
             four(q, A0, B0, Y0);
-            four(q + HS_THREADS, A1, B1, Y1);
+            four(q + NT, A1, B1, Y1);
         }
-        for (; q < q1; q += HS_THREADS) {
+        for (; q < q1; q += NT) {
             const float4 A = vp[q], Bv = vm[q];
             const float4 Y = y_is_minus ? Bv : (y_is_plus ? A : vy[q]);
             four(q, A, Bv, Y);
         }
     } else {
-        for (int64_t p = p0 + threadIdx.x; p < p1; p += HS_THREADS) one(mp[p], mm[p], my[p]);
+        for (int64_t p = p0 + threadIdx.x; p < p1; p += NT) one(mp[p], mm[p], my[p]);
     }
     // block reduction of the stats in a fixed order (deterministic)
-    __shared__ double r_sx[HS_THREADS / 32], r_sy[HS_THREADS / 32];
-    __shared__ uint32_t r_n[3][HS_THREADS / 32];
+    __shared__ double r_sx[NT / 32], r_sy[NT / 32];
+    __shared__ uint32_t r_n[3][NT / 32];
 #pragma unroll
     for (int d = 16; d > 0; d >>= 1) {
         n_in += __shfl_down_sync(0xffffffffu, n_in, d);
@@ -112,7 +113,7 @@ __global__ void __launch_bounds__(HS_THREADS, HS_MINB) k_hess(const float *__res
     __syncthreads();
     if (threadIdx.x == 0) {
         pcmd_hess_stats st = {0, 0, 0, 0, 0.0, 0.0};
-        for (int w = 0; w < HS_THREADS / 32; ++w) {
+        for (int w = 0; w < NT / 32; ++w) {
             st.n_in += r_n[0][w]; st.n_out += r_n[1][w]; st.n_bad += r_n[2][w];
             st.sum_x += r_sx[w]; st.sum_y += r_sy[w];
         }
@@ -122,9 +123,9 @@ __global__ void __launch_bounds__(HS_THREADS, HS_MINB) k_hess(const float *__res
     }
     if (SMEM) {
         if (gridDim.x == 1) {       // the only block of this diagram: plain stores, no memset needed
-            for (int t = threadIdx.x; t < nbins; t += HS_THREADS) gh[t] = sh[t];
+            for (int t = threadIdx.x; t < nbins; t += NT) gh[t] = sh[t];
         } else {
-            for (int t = threadIdx.x; t < nbins; t += HS_THREADS) {
+            for (int t = threadIdx.x; t < nbins; t += NT) {
                 uint32_t v = sh[t];
                 if (v) atomicAdd(&gh[t], v);
             }
@@ -158,6 +159,43 @@ __global__ void k_hess_stats(const pcmd_hess_stats *__restrict__ part, int nblk,
     }
 }
 
+// Memset (when several blocks share a diagram), k_hess and k_hess_stats for a given geometry; `parts` is the scratch
+// for the per-block partial statistics (the ctx's, or the fixed array of pcmd_hess_noalloc).
+static int hess_run(pcmd_ctx *c, const float *d_mag, int n_models, int nblk, int64_t ppb, uint32_t *d_hess,
+                    pcmd_hess_stats *parts, pcmd_hess_stats *d_stats, cudaStream_t s) {
+    int maxbins = 0;
+    for (int h = 0; h < c->n_hess; ++h) maxbins = max(maxbins, c->hess[h].nx * c->hess[h].ny);
+    const size_t smem = ((size_t)maxbins + 2) * sizeof(uint32_t);      // + the two spare counters
+    if (!(nblk == 1 && smem <= 200 * 1024))    // a single block per diagram stores its histogram itself
+        PCMD_CUDA(c, cudaMemsetAsync(d_hess, 0, (size_t)n_models * c->hess_bins * sizeof(uint32_t), s));
+    dim3 grid(nblk, c->n_hess, n_models);
+    if (smem <= 200 * 1024) {
+        // a histogram that leaves room for one block per SM only (c5: 200 x 200 bins = 160 KB) takes 1024 threads:
+        // the same number of warps per SM as two 512-thread blocks
+        const bool wide = smem > 100 * 1024;
+        if (smem > 48 * 1024 && smem > c->smem_hess) {      // an attribute of the functions, not an allocation
+            PCMD_CUDA(c, cudaFuncSetAttribute(k_hess<true, HS_THREADS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+            PCMD_CUDA(c, cudaFuncSetAttribute(k_hess<true, 1024>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+            c->smem_hess = smem;
+        }
+        if (wide)
+            PCMD_CUDA(c, pcmd_launch_pdl((k_hess<true, 1024>), grid, dim3(1024), smem, s, d_mag, c->B, c->P, c->d_hess_spec,
+                                         c->n_hess, ppb, c->hess_bins, d_hess, parts, d_stats));
+        else
+            PCMD_CUDA(c, pcmd_launch_pdl((k_hess<true, HS_THREADS>), grid, dim3(HS_THREADS), smem, s, d_mag, c->B, c->P,
+                                         c->d_hess_spec, c->n_hess, ppb, c->hess_bins, d_hess, parts, d_stats));
+    } else {
+        PCMD_CUDA(c, pcmd_launch_pdl((k_hess<false, HS_THREADS>), grid, dim3(HS_THREADS), 0, s, d_mag, c->B, c->P,
+                                     c->d_hess_spec, c->n_hess, ppb, c->hess_bins, d_hess, parts, d_stats));
+    }
+    PCMD_LAUNCHED(c);
+    if (d_stats && nblk > 1) {
+        PCMD_CUDA(c, pcmd_launch_pdl(k_hess_stats, dim3(n_models * c->n_hess), dim3(32), 0, s, parts, nblk, d_stats));
+        PCMD_LAUNCHED(c);
+    }
+    return PCMD_OK;
+}
+
 int pcmd_launch_hess(pcmd_ctx *c, const float *d_mag, int n_models, uint32_t *d_hess,
                      pcmd_hess_stats *d_stats, cudaStream_t s) {
     // Pixels per block: at least HS_PIX_PER_BLOCK (a block zeroes and flushes a whole private histogram, so long
@@ -177,29 +215,7 @@ int pcmd_launch_hess(pcmd_ctx *c, const float *d_mag, int n_models, uint32_t *d_
         PCMD_CUDA(c, cudaMalloc(&c->d_hpart, need * sizeof(pcmd_hess_stats)));
         c->hpart_cap = need;
     }
-    int maxbins = 0;
-    for (int h = 0; h < c->n_hess; ++h) maxbins = max(maxbins, c->hess[h].nx * c->hess[h].ny);
-    size_t smem = ((size_t)maxbins + 2) * sizeof(uint32_t);      // + the two spare counters
-    if (!(nblk == 1 && smem <= 200 * 1024))    // a single block per diagram stores its histogram itself
-        PCMD_CUDA(c, cudaMemsetAsync(d_hess, 0, (size_t)n_models * c->hess_bins * sizeof(uint32_t), s));
-    dim3 grid(nblk, c->n_hess, n_models);
-    if (smem <= 200 * 1024) {
-        if (smem > 48 * 1024 && smem > c->smem_hess) {
-            PCMD_CUDA(c, cudaFuncSetAttribute(k_hess<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-            c->smem_hess = smem;
-        }
-        pcmd_launch_pdl((k_hess<true>), grid, dim3(HS_THREADS), smem, s, d_mag, c->B, c->P, c->d_hess_spec, c->n_hess, ppb,
-                                                    c->hess_bins, d_hess, c->d_hpart, d_stats);
-    } else {
-        pcmd_launch_pdl((k_hess<false>), grid, dim3(HS_THREADS), 0, s, d_mag, c->B, c->P, c->d_hess_spec, c->n_hess, ppb,
-                                                  c->hess_bins, d_hess, c->d_hpart, d_stats);
-    }
-    PCMD_LAUNCHED(c);
-    if (d_stats && nblk > 1) {
-        pcmd_launch_pdl(k_hess_stats, dim3(n_models * c->n_hess), dim3(32), 0, s, c->d_hpart, nblk, d_stats);
-        PCMD_LAUNCHED(c);
-    }
-    return PCMD_OK;
+    return hess_run(c, d_mag, n_models, nblk, ppb, d_hess, c->d_hpart, d_stats, s);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -353,29 +369,9 @@ extern "C" int pcmd_hess_noalloc(pcmd_ctx *c, const float *d_mag, int32_t n_mode
     if ((int64_t)n_models * c->n_hess * nblk > PCMD_HESS_NOALLOC_MAX_PARTS) return PCMD_ELIMIT;
     pcmd_hess_stats *parts = nullptr;
     PCMD_CUDA(c, hess_noalloc_addr(&parts));
-    int maxbins = 0;
-    for (int h = 0; h < c->n_hess; ++h) maxbins = max(maxbins, c->hess[h].nx * c->hess[h].ny);
-    const size_t smem = ((size_t)maxbins + 2) * sizeof(uint32_t);      // + the two spare counters
     PCMD_PROF(c, 4, s);
-    if (!(nblk == 1 && smem <= 200 * 1024))
-        PCMD_CUDA(c, cudaMemsetAsync(d_hess, 0, (size_t)n_models * c->hess_bins * sizeof(uint32_t), s));
-    dim3 grid(nblk, c->n_hess, n_models);
-    if (smem <= 200 * 1024) {
-        if (smem > 48 * 1024 && smem > c->smem_hess) {      // an attribute of the function, not an allocation
-            PCMD_CUDA(c, cudaFuncSetAttribute(k_hess<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-            c->smem_hess = smem;
-        }
-        pcmd_launch_pdl((k_hess<true>), grid, dim3(HS_THREADS), smem, s, d_mag, c->B, c->P, c->d_hess_spec, c->n_hess, ppb,
-                                                    c->hess_bins, d_hess, parts, d_stats);
-    } else {
-        pcmd_launch_pdl((k_hess<false>), grid, dim3(HS_THREADS), 0, s, d_mag, c->B, c->P, c->d_hess_spec, c->n_hess, ppb,
-                                                  c->hess_bins, d_hess, parts, d_stats);
-    }
-    PCMD_LAUNCHED(c);
-    if (d_stats && nblk > 1) {
-        pcmd_launch_pdl(k_hess_stats, dim3(n_models * c->n_hess), dim3(32), 0, s, parts, nblk, d_stats);
-        PCMD_LAUNCHED(c);
-    }
+    const int rc = hess_run(c, d_mag, n_models, nblk, ppb, d_hess, parts, d_stats, s);
+    if (rc) return rc;
     PCMD_PROF(c, 5, s);
     return PCMD_OK;
 }
