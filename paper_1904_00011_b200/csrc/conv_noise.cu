@@ -35,7 +35,7 @@ __device__ __forceinline__ void noise_mag_epilogue(const CvArgs &a, const float 
                                                    int lx, int m, int b, int mb);
 
 __global__ void __launch_bounds__(CV_TX * CV_ROWS) k_conv_noise(const CvArgs a) {
-    pdl_enter();
+    pdl_enter<PDL_EARLY_CONV>();
     extern __shared__ float sm[];
     const int K = a.K, r = (K - 1) / 2, N = a.N;
     const int TW = CV_TX + K - 1, TH = CV_TY + K - 1;
@@ -95,7 +95,7 @@ __global__ void __launch_bounds__(CV_TX * CV_ROWS) k_conv_noise(const CvArgs a) 
 // memory, then the column pass: 2K FMAs per output instead of K^2.  Same tile, halo and epilogue.
 template <int KT>
 __global__ void __launch_bounds__(CV_TX * CV_ROWS) k_conv_noise_sep(const CvArgs a) {
-    pdl_enter();
+    pdl_enter<PDL_EARLY_CONV>();
     extern __shared__ float sm[];
     const int K = KT ? KT : a.K, r = (K - 1) / 2, N = a.N;
     const int TW = CV_TX + K - 1, TH = CV_TY + K - 1;
@@ -290,7 +290,7 @@ __device__ __forceinline__ float noise_mag_one(const Cv2Args &a, float Gi, uint3
 // NOISE = false: no shot / read noise and no Poisson sky (stage 5 is the magnitude only): a leaner instance
 template <int K, bool VEC, bool NOISE>
 __global__ void __launch_bounds__(C2_THREADS, (NOISE ? 4 : C2_MINB_CLEAN)) k_conv2(const Cv2Args a) {
-    pdl_enter();
+    pdl_enter<PDL_EARLY_CONV>();
     constexpr int R = (K - 1) / 2, RA = (R + 3) & ~3, OFF = RA - R;
     constexpr int SW = C2_TW + 2 * RA;            // halo-tile row stride (floats), a multiple of 4
     constexpr int SH = C2_TH + K - 1;             // halo-tile rows

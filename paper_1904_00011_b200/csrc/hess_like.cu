@@ -20,7 +20,7 @@ __global__ void __launch_bounds__(NT, (NT == HS_THREADS ? HS_MINB : 1)) k_hess(c
                                                      int64_t bins_total, uint32_t *__restrict__ hess,
                                                      pcmd_hess_stats *__restrict__ part,
                                                      pcmd_hess_stats *__restrict__ stats_out) {
-    pdl_enter();
+    pdl_enter<PDL_EARLY_HESS>();
     extern __shared__ uint32_t sh[];
     const int h = blockIdx.y, m = blockIdx.z;
     const DevHess S = specs[h];
@@ -135,7 +135,7 @@ __global__ void __launch_bounds__(NT, (NT == HS_THREADS ? HS_MINB : 1)) k_hess(c
 
 __global__ void k_hess_stats(const pcmd_hess_stats *__restrict__ part, int nblk,
                              pcmd_hess_stats *__restrict__ out) {
-    pdl_enter();
+    pdl_enter<PDL_EARLY_HESS>();
     // one warp per (model, hess): lane l adds partials l, l+32, ... in order, then a shuffle tree
     // (a fixed order: deterministic sums)
     const pcmd_hess_stats *p = part + (size_t)blockIdx.x * nblk;
@@ -255,7 +255,7 @@ __global__ void __launch_bounds__(LL_THREADS) k_loglike(const uint32_t *__restri
                                                         int64_t bins_total, int mode, double m_floor,
                                                         const double *__restrict__ lfact,
                                                         double *__restrict__ out) {
-    pdl_enter();
+    pdl_enter<PDL_EARLY_LIKE>();
     __shared__ double scratch[LL_THREADS / 32];
     const int m = blockIdx.x;
     double total = 0.0;

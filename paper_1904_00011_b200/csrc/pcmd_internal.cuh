@@ -183,7 +183,7 @@ struct pcmd_ctx {
 
 // Programmatic dependent launch (PDL) -------------------------------------------------------
 // The kernels of one evaluation form a chain on the caller's stream, and on small jobs (c1: 64 x 64 pixels) the
-// launch latency between them is a large part of the step.  Every kernel of the chain starts with pdl_enter():
+// launch latency between them is a large part of the step.  Every kernel of the chain starts with pdl_enter<EARLY>():
 // griddepcontrol.wait (returns once the previous kernel of the stream has completed and its writes are visible;
 // a no-op for a kernel launched without the attribute) followed by griddepcontrol.launch_dependents (lets the
 // NEXT kernel, if it was launched with the attribute, be set up and made resident while this one runs; it then
@@ -191,10 +191,39 @@ struct pcmd_ctx {
 // anything else.  pcmd_launch_pdl launches with cudaLaunchAttributeProgrammaticStreamSerialization; only
 // kernels that begin with pdl_enter() may be launched through it.  PCMD_NO_PDL=1 in the environment switches
 // the attribute off (plain stream order).
+// EARLY = false leaves the trigger to the kernel's exit: the warps of an early-resident dependent poll in their wait
+// and take issue slots from the kernel that is still running, which costs more than the hidden launch latency when
+// that kernel is a handful of latency-bound threads (k_points: a serial fp64 recurrence per thread; measured 3 us of
+// stage 1 in every configuration).  Per-kernel switches (PDL_EARLY_*) below.
+template <bool EARLY>
 __device__ __forceinline__ void pdl_enter() {
     asm volatile("griddepcontrol.wait;" ::: "memory");
-    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+    if (EARLY) asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
 }
+#ifndef PDL_EARLY_POINTS
+#define PDL_EARLY_POINTS 0
+#endif
+#ifndef PDL_EARLY_SORT
+#define PDL_EARLY_SORT 1
+#endif
+#ifndef PDL_EARLY_EMIT
+#define PDL_EARLY_EMIT 1
+#endif
+#ifndef PDL_EARLY_STAGE2
+#define PDL_EARLY_STAGE2 1
+#endif
+#ifndef PDL_EARLY_REDUCE
+#define PDL_EARLY_REDUCE 1
+#endif
+#ifndef PDL_EARLY_CONV
+#define PDL_EARLY_CONV 1
+#endif
+#ifndef PDL_EARLY_HESS
+#define PDL_EARLY_HESS 1
+#endif
+#ifndef PDL_EARLY_LIKE
+#define PDL_EARLY_LIKE 1
+#endif
 int pcmd_pdl_enabled();     // api.cu
 template <typename... KA, typename... A>
 static inline cudaError_t pcmd_launch_pdl(void (*kern)(KA...), dim3 grid, dim3 block, size_t smem, cudaStream_t s,

@@ -245,7 +245,7 @@ __constant__ uint32_t c_s2_group_cost[S2_NCLASS] = {S2_COST_G, S2_COST_D9, S2_CO
 __global__ void __launch_bounds__(1024) k_group_sort(const uint8_t *__restrict__ cls_all, int Jpad,
                                                      int64_t arena_cap, uint32_t *__restrict__ pos_all,
                                                      ModelPlan *__restrict__ plan_all) {
-    pdl_enter();
+    pdl_enter<PDL_EARLY_SORT>();
     __shared__ uint32_t wcnt[32][S2_NCLASS];
     __shared__ uint32_t count[S2_NCLASS + 1], carry[S2_NCLASS], cls_start[S2_NCLASS + 1];
     const int m = blockIdx.x, n_groups = Jpad >> 2;
@@ -338,7 +338,7 @@ __global__ void __launch_bounds__(128) k_points(const DevModel *__restrict__ mdl
                          double *__restrict__ qbuf, int64_t cap, uint32_t *__restrict__ tab_all,
                          uint32_t *__restrict__ alloc, PointRec *__restrict__ rec_out,
                          uint8_t *__restrict__ gcls_out, int32_t *status) {
-    pdl_enter();
+    pdl_enter<PDL_EARLY_POINTS>();
     extern __shared__ double w[];  // [Z]
     const int m = blockIdx.y;
     const DevModel M = mdl[m];
@@ -443,7 +443,7 @@ __global__ void __launch_bounds__(256) k_group_emit(const PointRec *__restrict__
                                                     const uint32_t *__restrict__ pos_all,
                                                     const ModelPlan *__restrict__ plan_all, GroupRec *__restrict__ grp_all,
                                                     uint32_t *__restrict__ arena_all, int64_t arena_cap) {
-    pdl_enter();
+    pdl_enter<PDL_EARLY_EMIT>();
     const int m = blockIdx.y, n_groups = Jpad >> 2, lane = threadIdx.x & 31;
     const int g = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
     if (g >= n_groups) return;

@@ -439,7 +439,7 @@ __device__ __forceinline__ void s2_issue(const S2Args &a, S2Shared &sh, GroupRec
 // ---- the persistent kernel ----------------------------------------------------------------------
 template <int NB, bool COUNTS>
 __global__ void __launch_bounds__(S2_THREADS, S2_MINB) k_stage2(const S2Args a) {
-    pdl_enter();
+    pdl_enter<PDL_EARLY_STAGE2>();
     extern __shared__ __align__(128) unsigned char s2_smem[];
     GroupRec *sbuf = reinterpret_cast<GroupRec *>(s2_smem);                                     // [S2_NST][S2_CHUNK]
     uint32_t *stab = reinterpret_cast<uint32_t *>(s2_smem + (size_t)S2_NST * S2_CHUNK * sizeof(GroupRec));   // [S2_NST][S2_TABW]
@@ -577,7 +577,7 @@ struct RdArgs {
 };
 
 __global__ void __launch_bounds__(256) k_reduce_dust(const RdArgs a) {
-    pdl_enter();
+    pdl_enter<PDL_EARLY_REDUCE>();
     const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (idx >= a.P * a.n_models) return;
     const int m = (int)(idx / a.P);
