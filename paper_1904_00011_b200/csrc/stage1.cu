@@ -243,7 +243,7 @@ __device__ __forceinline__ int point_class(const PointRec &r, const uint32_t *__
 __constant__ uint32_t c_s2_group_cost[S2_NCLASS] = {S2_COST_G, S2_COST_D9, S2_COST_D8, S2_COST_D7, S2_COST_D6, S2_COST_D5, S2_COST_S4, S2_COST_S3,
                                                     S2_COST_L4, S2_COST_L2, S2_COST_L1, S2_COST_L0};
 __global__ void __launch_bounds__(1024) k_group_sort(const uint8_t *__restrict__ cls_all, int Jpad,
-                                                     int64_t arena_cap, uint32_t *__restrict__ pos_all,
+                                                     int64_t arena_cap, int n_seg, uint32_t *__restrict__ pos_all,
                                                      ModelPlan *__restrict__ plan_all) {
     pdl_enter<PDL_EARLY_SORT>();
     __shared__ uint32_t wcnt[32][S2_NCLASS];
@@ -295,6 +295,16 @@ __global__ void __launch_bounds__(1024) k_group_sort(const uint8_t *__restrict__
             if (need <= arena_cap || first_d > S2_CLS_S3) break;
             first_d++;
         }
+        // A small model (c1: 64 groups) cut into full-size chunks has fewer chunks than the n_seg segments stage 2
+        // wants per tile (a segment is at least one chunk), and its few work units then run their groups one after
+        // the other: chunks are shrunk to about 1/n_seg of the model's cost.  Models of the larger configurations
+        // (cost / n_seg above a full chunk) keep their chunk sizes.
+        uint32_t group_cost_total = 0;        // 32-bit like the plan's cost_total
+        for (int c = 0; c < S2_NCLASS; ++c) {
+            const bool demoted_c = c >= S2_CLS_D9 && c <= S2_CLS_S3 && !(c >= first_d && c <= S2_CLS_S3);
+            group_cost_total += count[c] * c_s2_group_cost[demoted_c ? 0 : c];
+        }
+        const uint32_t chunk_cost_target = group_cost_total / (uint32_t)max(n_seg, 1);
         int64_t off = 0;
         int32_t chunks = 0;
         uint32_t cost = 0, cmax = 0;
@@ -305,7 +315,9 @@ __global__ void __launch_bounds__(1024) k_group_sort(const uint8_t *__restrict__
             if (in_arena) { t.arena_off[c] = off; off += stride[c] * (int64_t)count[c]; }
             const bool demoted = c >= S2_CLS_D9 && c <= S2_CLS_S3 && !in_arena;
             t.run_cls[c] = demoted ? 0 : c;
-            const int cg = in_arena ? min((int)(S2_TABW / stride[c]), S2_CHUNK) : S2_CHUNK;     // groups per chunk
+            int cg = in_arena ? min((int)(S2_TABW / stride[c]), S2_CHUNK) : S2_CHUNK;     // groups per chunk
+            if (chunk_cost_target < (uint32_t)cg * c_s2_group_cost[t.run_cls[c]])
+                cg = (int)max(chunk_cost_target / c_s2_group_cost[t.run_cls[c]], 1u);
             t.chunk_groups[c] = cg;
             t.chunk_cost[c] = (uint32_t)cg * c_s2_group_cost[t.run_cls[c]] + S2_COST_CHUNK;
             const int n = (int)count[c], nch = (n + cg - 1) / cg;
@@ -523,7 +535,7 @@ int pcmd_launch_stage1(pcmd_ctx *c, int n_models, cudaStream_t s) {
         c->Jpad, c->B, c->mdf_cut, c->zp[0], c->zp[1], c->zp[2], c->zp[3], c->d_mdfw, c->d_lambda, c->d_q,
         c->cap_raw, c->d_tab, c->d_alloc, c->d_rec, c->d_gcls, c->d_status);
     PCMD_LAUNCHED(c);
-    pcmd_launch_pdl(k_group_sort, dim3(n_models), dim3(1024), 0, s, c->d_gcls, c->Jpad, c->arena_cap, c->d_gpos, c->d_plan);
+    pcmd_launch_pdl(k_group_sort, dim3(n_models), dim3(1024), 0, s, c->d_gcls, c->Jpad, c->arena_cap, c->n_seg, c->d_gpos, c->d_plan);
     PCMD_LAUNCHED(c);
     pcmd_launch_pdl(k_group_emit, dim3((n_groups + 7) / 8, n_models), dim3(256), 0, s, c->d_rec, c->d_tab, c->cap_raw, c->Jpad, c->d_gcls,
                                                                     c->d_gpos, c->d_plan, c->d_grp, c->d_arena,
