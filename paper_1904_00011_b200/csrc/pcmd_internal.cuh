@@ -210,7 +210,7 @@ __device__ __forceinline__ void pdl_enter() {
 #define PDL_EARLY_EMIT 1
 #endif
 #ifndef PDL_EARLY_STAGE2
-#define PDL_EARLY_STAGE2 1
+#define PDL_EARLY_STAGE2 0        // k_reduce_dust blocks that fill in next to the last running k_stage2 blocks poll beside them (c1: -1.5 us)
 #endif
 #ifndef PDL_EARLY_REDUCE
 #define PDL_EARLY_REDUCE 1
